@@ -1,0 +1,173 @@
+/*
+ * ws.h -- C ABI of the B200-native performer hot path of Wan-Streamer v0.2
+ *         (arxiv/paper_2607_04443; citations are PAPER.md line numbers).
+ *
+ * One Ulysses performer rank's single-GPU share of a 160 ms streaming unit:
+ *
+ *   ws_kv_cache_write      "each performer rank writes incoming K/V into a pre-sharded local
+ *                           cache"
+ *   ws_seq_to_head /       the rank-local halves of the "Ulysses all-to-all/gather collectives
+ *   ws_head_to_seq          around attention"
+ *   ws_block_causal_attn   the unit's latent query tokens attend, "coordinated by block-causal
+ *                           attention", to the cached K/V conditioning plus the unit's own K/V
+ *                                                                   PAPER.md:25, :73, :79
+ *   ws_unit_forward_host   the same path for one unit fed from HOST buffers (end-to-end entry)
+ *
+ * Conventions (all functions)
+ *   - Return value: WS_OK (0) or a negative ws_status.  On any error NOTHING is launched and no
+ *     output byte is modified.  WS_ERR_CUDA keeps the cudaError_t in ws_last_cuda_error().
+ *   - Pointers documented "device" are CUDA device pointers OWNED BY THE CALLER and borrowed
+ *     until the stream-ordered work completes.  Pointers documented "host" are read during the
+ *     call only.  Device pointers must be 16-byte aligned and d * sizeof(element) a multiple of
+ *     16 (WS_ERR_ALIGNMENT otherwise).
+ *   - No allocation, no synchronisation, no host read of device data: every call is legal
+ *     inside CUDA stream capture.  `stream` is a cudaStream_t passed as void* (NULL = default).
+ *   - Batch is 1 (fold a batch into heads).  Layouts are dense row-major with the last index
+ *     fastest: token-major [L, H, d] for Q / K_new / V_new / O / slices, head-major
+ *     [H, capacity, d] for the cache (private to the rank; reading R5).
+ *   - There is no CPU fallback: without a CUDA device every launching call fails.
+ */
+#ifndef WS_H_
+#define WS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define WS_VERSION 100 /* major*10000 + minor*100 + patch */
+
+typedef enum { WS_DTYPE_BF16 = 0, WS_DTYPE_F32 = 1 } ws_dtype;
+
+typedef enum {
+  WS_OK = 0,
+  WS_ERR_INVALID_ARG = -1,  /* NULL pointer, non-positive size, malformed mask, H % P != 0 ...   */
+  WS_ERR_UNSUPPORTED = -2,  /* dtype / head_dim / mask size this build has no kernel for         */
+  WS_ERR_ALIGNMENT = -3,    /* a device pointer or row pitch is not 16-byte aligned              */
+  WS_ERR_OUT_OF_RANGE = -4, /* row_offset+n_rows > capacity, cache_len > capacity, kv_visible > cache_len+Ln */
+  WS_ERR_OVERLAP = -5,      /* source and destination byte ranges intersect                      */
+  WS_ERR_WORKSPACE = -6,    /* workspace NULL or smaller than ws_block_causal_attn_workspace_bytes */
+  WS_ERR_CUDA = -7          /* CUDA runtime/driver error; see ws_last_cuda_error()               */
+} ws_status;
+
+/* Limits of this build. */
+#define WS_MAX_MASK_BLOCKS 128 /* n_blocks of a ws_block_mask */
+
+/* ------------------------------------------------------------------------------------------------
+ * a1. KV cache write
+ *
+ *   cache[h, row_offset + r, :] = src[r, head_begin + h, :]   0 <= h < H, 0 <= r < n_rows
+ *   for K and for V; every other cache byte is untouched.
+ *
+ *   k_cache, v_cache : device, [H, capacity, d]   (written)
+ *   k_src, v_src     : device, [n_rows, H_src, d] (read) -- the thinker's broadcast slice with all
+ *                      H_src heads; this rank keeps heads [head_begin, head_begin + H).
+ *   n_rows == 0 is a no-op (WS_OK).  Errors: OUT_OF_RANGE if row_offset < 0 or
+ *   row_offset + n_rows > capacity; INVALID_ARG if head_begin < 0 or head_begin + H > H_src;
+ *   OVERLAP if a source range intersects a cache range.
+ * ---------------------------------------------------------------------------------------------- */
+int ws_kv_cache_write(void* k_cache, void* v_cache, int64_t capacity, int32_t H, int32_t d,
+                      const void* k_src, const void* v_src, int32_t n_rows, int32_t H_src,
+                      int32_t head_begin, int64_t row_offset, ws_dtype dt, void* stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * a2 / a4. Ulysses-local relayouts
+ *
+ *   With Hp = H / P heads per rank-group:
+ *   ws_seq_to_head:  dst[g, t, c, :] = src[t, (g0 + g) * Hp + c, :]
+ *   ws_head_to_seq:  dst[t, (g0 + g) * Hp + c, :] = src[g, t, c, :]   (other heads of dst untouched)
+ *   for 0 <= g < G, 0 <= t < n_tok, 0 <= c < Hp.  They are exact inverses on the selected heads.
+ *
+ *   token-major side : device, [n_tok, H, d]       head-major side : device, [G, n_tok, Hp, d]
+ *   G = 1 with g0 = rank is what one rank needs after all-to-all #1 when all sequence shards are
+ *   local (config 4); G = P packs every peer's chunk (the send buffer of a real all-to-all).
+ *   Errors: INVALID_ARG if P <= 0, H % P != 0, g0 < 0, G < 0 or g0 + G > P; OVERLAP if src and dst
+ *   intersect.  n_tok == 0 or G == 0 is a no-op.
+ * ---------------------------------------------------------------------------------------------- */
+int ws_seq_to_head(void* dst, const void* src, int64_t n_tok, int32_t H, int32_t d, int32_t P,
+                   int32_t g0, int32_t G, ws_dtype dt, void* stream);
+int ws_head_to_seq(void* dst, const void* src, int64_t n_tok, int32_t H, int32_t d, int32_t P,
+                   int32_t g0, int32_t G, ws_dtype dt, void* stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * a3. Block-causal unit attention
+ *
+ *   Key timeline: j < cache_len is cache row j; cache_len <= j < cache_len + Ln is row
+ *   j - cache_len of k_new / v_new.  Query block b covers rows [q_block_end[b-1], q_block_end[b])
+ *   (q_block_end[-1] = 0) and sees the keys j < kv_visible[b]:
+ *
+ *     O[i, h, :] = sum_{j < kv_visible[b(i)]} softmax_j(softmax_scale * q[i,h,:] . k_j[h,:]) v_j[h,:]
+ *     lse[h, i]  = natural-log-sum-exp of the visible scaled logits
+ *     kv_visible[b] == 0  ->  O row = 0, lse = -inf (no NaN).
+ *
+ *   A streaming unit is one block (bidirectional inside the unit, causal across units).
+ *
+ *   out      : device, [Lq, H, d], same dtype as q (written)
+ *   lse      : device, float [H, Lq], or NULL
+ *   q        : device, [Lq, H, d]
+ *   k_cache, v_cache : device, [H, capacity, d]; rows [0, cache_len) are valid and must be finite
+ *   k_new, v_new     : device, [Ln, H, d]; NULL iff Ln == 0
+ *   mask     : host; q_block_end strictly increasing with last == Lq; kv_visible non-decreasing,
+ *              0 <= kv_visible[b] <= cache_len + Ln; n_blocks <= WS_MAX_MASK_BLOCKS
+ *   workspace: device, >= ws_block_causal_attn_workspace_bytes(...) bytes, 256-byte aligned;
+ *              contents are scratch (split-KV partials; BF16 staging for WS_DTYPE_F32)
+ *
+ *   Arithmetic: BF16 operands, FP32 accumulation (tcgen05), FP32 softmax, probabilities rounded
+ *   to BF16 before P.V.  WS_DTYPE_F32 inputs are rounded to BF16 on the device first and the
+ *   output is written as FP32 (config 1; reading R9).  Supported: d in {64, 128}.
+ *   Errors: UNSUPPORTED (d, dt, n_blocks), INVALID_ARG (malformed mask, NULLs), OUT_OF_RANGE
+ *   (cache_len > capacity, kv_visible > cache_len + Ln), WORKSPACE, ALIGNMENT, CUDA.
+ * ---------------------------------------------------------------------------------------------- */
+typedef struct ws_block_mask {
+  int32_t n_blocks;
+  const int32_t* q_block_end; /* host */
+  const int32_t* kv_visible;  /* host */
+} ws_block_mask;
+
+size_t ws_block_causal_attn_workspace_bytes(int32_t Lq, int32_t H, int32_t d, int64_t kv_total, ws_dtype dt);
+
+int ws_block_causal_attn(void* out, float* lse, const void* q, const void* k_cache, const void* v_cache,
+                         int64_t capacity, int64_t cache_len, const void* k_new, const void* v_new, int32_t Ln,
+                         int32_t H, int32_t d, int32_t Lq, const ws_block_mask* mask, float softmax_scale,
+                         void* workspace, size_t workspace_bytes, ws_dtype dt, void* stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * a5. One unit end to end from HOST buffers ("receive the current K/V slice, update
+ *     their local shards of the full-history cache, and run ... denoising for the next unit").
+ *
+ *   Stream-ordered on `stream`:  H2D copies of the slice and of every step's Q/K_new/V_new ->
+ *   ws_kv_cache_write (if n_slice_rows > 0) -> n_steps x ws_block_causal_attn (step s uses
+ *   q_host[s], k_new_host[s], v_new_host[s]; the mask is the single block "all Lq rows see
+ *   cache_len_after + Ln keys") -> D2H copy of every step's output into out_host[s].
+ *   The call does not synchronise; the caller synchronises the stream before reading out_host.
+ *
+ *   k_cache, v_cache : device [H, capacity, d]      (the persistent local cache)
+ *   k_slice_host, v_slice_host : host (pinned for async copies) [n_slice_rows, H, d], written at
+ *                      row_offset; cache_len_after = valid rows once the slice is in
+ *   q_host, k_new_host, v_new_host : host [n_steps][Lq | Ln, H, d] contiguous over steps
+ *   out_host         : host [n_steps][Lq, H, d]
+ *   staging          : device scratch >= ws_unit_forward_host_staging_bytes(...) (inputs, outputs,
+ *                      attention workspace), 256-byte aligned
+ *   BF16 only.  Same error rules as the calls it is made of.
+ * ---------------------------------------------------------------------------------------------- */
+size_t ws_unit_forward_host_staging_bytes(int32_t Lq, int32_t Ln, int32_t H, int32_t d, int32_t n_slice_rows,
+                                          int64_t kv_total, int32_t n_steps);
+
+int ws_unit_forward_host(void* out_host, const void* q_host, const void* k_new_host, const void* v_new_host,
+                         int32_t Lq, int32_t Ln, int32_t n_steps, void* k_cache, void* v_cache, int64_t capacity,
+                         const void* k_slice_host, const void* v_slice_host, int32_t n_slice_rows, int64_t row_offset,
+                         int64_t cache_len_after, int32_t H, int32_t d, float softmax_scale, void* staging,
+                         size_t staging_bytes, void* stream);
+
+/* ---- utilities ---- */
+const char* ws_status_string(int status); /* static string, never NULL */
+int ws_version(void);                     /* WS_VERSION of the loaded library */
+int ws_last_cuda_error(void);             /* cudaError_t of the last WS_ERR_CUDA on this thread, else 0 */
+int ws_kernel_launch_count(void);         /* kernels this library has launched in this process so far */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WS_H_ */

@@ -1,0 +1,217 @@
+"""ctypes binding of libws.so (include/ws.h): same names, argument marshalling only.
+
+Tensors are torch CUDA tensors (PyTorch is used for device memory and streams, nothing else);
+every step of the path runs in the library's own kernels.  There is NO fallback: if libws.so is
+missing, or a tensor is not on a CUDA device, the call raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import torch
+
+DTYPE_BF16 = 0
+DTYPE_F32 = 1
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_PKG, "libws.so")
+_lib = None
+
+EXPORTS = (
+    "ws_kv_cache_write", "ws_seq_to_head", "ws_head_to_seq", "ws_block_causal_attn_workspace_bytes",
+    "ws_block_causal_attn", "ws_unit_forward_host_staging_bytes", "ws_unit_forward_host", "ws_status_string",
+    "ws_version", "ws_last_cuda_error", "ws_kernel_launch_count",
+)
+
+
+class WsError(RuntimeError):
+    def __init__(self, status: int, what: str):
+        self.status = status
+        msg = status_string(status)
+        if status == -7:
+            msg += f" [cudaError {load().ws_last_cuda_error()}]"
+        super().__init__(f"{what}: {msg}")
+
+
+class _BlockMask(ctypes.Structure):
+    _fields_ = [("n_blocks", ctypes.c_int32), ("q_block_end", ctypes.POINTER(ctypes.c_int32)),
+                ("kv_visible", ctypes.POINTER(ctypes.c_int32))]
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def load():
+    """Loads libws.so.  Raises (loudly) if it has not been built: there is no other path."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise RuntimeError(f"{_LIB_PATH} not found: build it with `python -m paper_2607_04443_b200.build` "
+                           "(there is no CPU or PyTorch fallback)")
+    lib = ctypes.CDLL(_LIB_PATH)
+    i32, i64, vp, sz, f32 = ctypes.c_int32, ctypes.c_int64, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_float
+    lib.ws_kv_cache_write.argtypes = [vp, vp, i64, i32, i32, vp, vp, i32, i32, i32, i64, ctypes.c_int, vp]
+    lib.ws_kv_cache_write.restype = ctypes.c_int
+    for fn in (lib.ws_seq_to_head, lib.ws_head_to_seq):
+        fn.argtypes = [vp, vp, i64, i32, i32, i32, i32, i32, ctypes.c_int, vp]
+        fn.restype = ctypes.c_int
+    lib.ws_block_causal_attn_workspace_bytes.argtypes = [i32, i32, i32, i64, ctypes.c_int]
+    lib.ws_block_causal_attn_workspace_bytes.restype = sz
+    lib.ws_block_causal_attn.argtypes = [vp, vp, vp, vp, vp, i64, i64, vp, vp, i32, i32, i32, i32,
+                                         ctypes.POINTER(_BlockMask), f32, vp, sz, ctypes.c_int, vp]
+    lib.ws_block_causal_attn.restype = ctypes.c_int
+    lib.ws_unit_forward_host_staging_bytes.argtypes = [i32, i32, i32, i32, i32, i64, i32]
+    lib.ws_unit_forward_host_staging_bytes.restype = sz
+    lib.ws_unit_forward_host.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp, i64, vp, vp, i32, i64, i64, i32, i32, f32,
+                                         vp, sz, vp]
+    lib.ws_unit_forward_host.restype = ctypes.c_int
+    lib.ws_status_string.argtypes = [ctypes.c_int]
+    lib.ws_status_string.restype = ctypes.c_char_p
+    for fn in (lib.ws_version, lib.ws_last_cuda_error, lib.ws_kernel_launch_count):
+        fn.argtypes = []
+        fn.restype = ctypes.c_int
+    _lib = lib
+    return lib
+
+
+def version() -> int:
+    return int(load().ws_version())
+
+
+def status_string(status: int) -> str:
+    return load().ws_status_string(int(status)).decode()
+
+
+def kernel_launch_count() -> int:
+    return int(load().ws_kernel_launch_count())
+
+
+def _dt(t: torch.Tensor) -> int:
+    if t.dtype == torch.bfloat16:
+        return DTYPE_BF16
+    if t.dtype == torch.float32:
+        return DTYPE_F32
+    raise TypeError(f"unsupported dtype {t.dtype}: the library moves/computes BF16 or FP32")
+
+
+def _dev(*tensors):
+    for t in tensors:
+        if t is None:
+            continue
+        if not t.is_cuda:
+            raise RuntimeError("ws: tensors must live on a CUDA device (no CPU fallback exists)")
+        if not t.is_contiguous():
+            raise ValueError("ws: tensors must be contiguous")
+
+
+def _p(t: Optional[torch.Tensor]):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def _stream(stream) -> ctypes.c_void_p:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+def _ok(rc: int, what: str):
+    if rc != 0:
+        raise WsError(rc, what)
+
+
+def kv_cache_write(k_cache, v_cache, k_src, v_src, head_begin: int = 0, row_offset: int = 0, stream=None):
+    """cache[h, row_offset + r, :] = src[r, head_begin + h, :] for K and V (ws.h a1)."""
+    _dev(k_cache, v_cache, k_src, v_src)
+    H, capacity, d = k_cache.shape
+    n_rows, H_src, d2 = k_src.shape
+    if d2 != d or v_cache.shape != k_cache.shape or v_src.shape != k_src.shape:
+        raise ValueError("ws_kv_cache_write: shape mismatch")
+    if not (k_cache.dtype == v_cache.dtype == k_src.dtype == v_src.dtype):
+        raise TypeError("ws_kv_cache_write: dtype mismatch")
+    rc = load().ws_kv_cache_write(_p(k_cache), _p(v_cache), capacity, H, d, _p(k_src), _p(v_src), n_rows, H_src, head_begin,
+                                  row_offset, _dt(k_cache), _stream(stream))
+    _ok(rc, "ws_kv_cache_write")
+
+
+def seq_to_head(dst, src, P: int, g0: int, G: int, stream=None):
+    """dst[g, t, c, :] = src[t, (g0 + g) * H/P + c, :]  (ws.h a2); src [n_tok, H, d]."""
+    _dev(dst, src)
+    n_tok, H, d = src.shape
+    if dst.dtype != src.dtype:
+        raise TypeError("ws_seq_to_head: dtype mismatch")
+    if P > 0 and H % P == 0 and tuple(dst.shape) != (G, n_tok, H // P, d):
+        raise ValueError("ws_seq_to_head: dst must be [G, n_tok, H/P, d]")
+    _ok(load().ws_seq_to_head(_p(dst), _p(src), n_tok, H, d, P, g0, G, _dt(src), _stream(stream)), "ws_seq_to_head")
+
+
+def head_to_seq(dst, src, P: int, g0: int, G: int, stream=None):
+    """dst[t, (g0 + g) * H/P + c, :] = src[g, t, c, :]  (ws.h a4); dst [n_tok, H, d]."""
+    _dev(dst, src)
+    n_tok, H, d = dst.shape
+    if dst.dtype != src.dtype:
+        raise TypeError("ws_head_to_seq: dtype mismatch")
+    if P > 0 and H % P == 0 and tuple(src.shape) != (G, n_tok, H // P, d):
+        raise ValueError("ws_head_to_seq: src must be [G, n_tok, H/P, d]")
+    _ok(load().ws_head_to_seq(_p(dst), _p(src), n_tok, H, d, P, g0, G, _dt(dst), _stream(stream)), "ws_head_to_seq")
+
+
+def block_causal_attn_workspace_bytes(Lq: int, H: int, d: int, kv_total: int, dtype=torch.bfloat16) -> int:
+    dt = DTYPE_BF16 if dtype == torch.bfloat16 else DTYPE_F32
+    return int(load().ws_block_causal_attn_workspace_bytes(Lq, H, d, kv_total, dt))
+
+
+def block_causal_attn(out, q, k_cache, v_cache, cache_len: int, k_new, v_new, q_block_end: Sequence[int],
+                      kv_visible: Sequence[int], softmax_scale: float, workspace, lse=None, stream=None):
+    """Block-causal unit attention (ws.h a3).  out/q [Lq,H,d]; caches [H,capacity,d]; k_new/v_new [Ln,H,d] or None."""
+    _dev(out, q, k_cache, v_cache, k_new, v_new, workspace, lse)
+    Lq, H, d = q.shape
+    capacity = k_cache.shape[1]
+    Ln = 0 if k_new is None else k_new.shape[0]
+    if out.shape != q.shape or out.dtype != q.dtype:
+        raise ValueError("ws_block_causal_attn: out must match q")
+    if tuple(k_cache.shape) != (H, capacity, d) or v_cache.shape != k_cache.shape:
+        raise ValueError("ws_block_causal_attn: cache must be [H, capacity, d]")
+    if k_new is not None and (tuple(k_new.shape) != (Ln, H, d) or v_new is None or v_new.shape != k_new.shape):
+        raise ValueError("ws_block_causal_attn: k_new/v_new must be [Ln, H, d]")
+    for t in (k_cache, v_cache, k_new, v_new):
+        if t is not None and t.dtype != q.dtype:
+            raise TypeError("ws_block_causal_attn: dtype mismatch")
+    if lse is not None and (lse.dtype != torch.float32 or tuple(lse.shape) != (H, Lq)):
+        raise ValueError("ws_block_causal_attn: lse must be float32 [H, Lq]")
+    n = len(q_block_end)
+    if len(kv_visible) != n:
+        raise ValueError("ws_block_causal_attn: mask arrays differ in length")
+    qe = (ctypes.c_int32 * n)(*[int(x) for x in q_block_end])
+    kv = (ctypes.c_int32 * n)(*[int(x) for x in kv_visible])
+    mask = _BlockMask(n, qe, kv)
+    rc = load().ws_block_causal_attn(_p(out), _p(lse), _p(q), _p(k_cache), _p(v_cache), capacity, int(cache_len), _p(k_new),
+                                     _p(v_new), Ln, H, d, Lq, ctypes.byref(mask), float(softmax_scale), _p(workspace),
+                                     workspace.numel() * workspace.element_size(), _dt(q), _stream(stream))
+    _ok(rc, "ws_block_causal_attn")
+
+
+def unit_forward_host_staging_bytes(Lq, Ln, H, d, n_slice_rows, kv_total, n_steps) -> int:
+    return int(load().ws_unit_forward_host_staging_bytes(Lq, Ln, H, d, n_slice_rows, kv_total, n_steps))
+
+
+def unit_forward_host(out_host, q_host, k_new_host, v_new_host, k_cache, v_cache, k_slice_host, v_slice_host,
+                      row_offset: int, cache_len_after: int, softmax_scale: float, staging, stream=None):
+    """One unit from HOST (pinned CPU) tensors (ws.h a5).  q_host/out_host [n_steps, Lq, H, d] BF16 CPU tensors,
+    k_new_host/v_new_host [n_steps, Ln, H, d] or None, slices [n_rows, H, d] or None; caches and staging on the GPU."""
+    _dev(k_cache, v_cache, staging)
+    for t in (out_host, q_host, k_new_host, v_new_host, k_slice_host, v_slice_host):
+        if t is not None and (t.is_cuda or not t.is_contiguous() or t.dtype != torch.bfloat16):
+            raise ValueError("ws_unit_forward_host: host tensors must be contiguous BF16 CPU tensors")
+    n_steps, Lq, H, d = q_host.shape
+    Ln = 0 if k_new_host is None else k_new_host.shape[1]
+    n_rows = 0 if k_slice_host is None else k_slice_host.shape[0]
+    capacity = k_cache.shape[1]
+    rc = load().ws_unit_forward_host(_p(out_host), _p(q_host), _p(k_new_host), _p(v_new_host), Lq, Ln, n_steps, _p(k_cache),
+                                     _p(v_cache), capacity, _p(k_slice_host), _p(v_slice_host), n_rows, int(row_offset),
+                                     int(cache_len_after), H, d, float(softmax_scale), _p(staging),
+                                     staging.numel() * staging.element_size(), _stream(stream))
+    _ok(rc, "ws_unit_forward_host")

@@ -1,0 +1,715 @@
+// ws_attn.cu -- block-causal unit attention for sm_100a (include/ws.h a3).
+//
+// Flash-style forward pass written directly on the Blackwell primitives:
+//   * K/V tiles (128 keys x d) and the two 128-row Q tiles of a CTA are staged in shared memory
+//     by TMA (cp.async.bulk.tensor, 128-byte swizzle) through a 5-slot mbarrier ring;
+//   * S = Q K^T and O += P V run on the 5th-gen tensor cores (tcgen05.mma, BF16 in, FP32
+//     accumulate) with S, P and O living in TMEM: S0,S1 (128 columns each), O0,O1 (d columns
+//     each); P overwrites S in place as packed BF16 and is fed back as the TMEM A operand;
+//   * the online softmax is done by two 128-thread warpgroups, one per Q tile, one thread per
+//     query row (tcgen05.ld 32x32b gives each thread its row: no shuffles), exp2 with the scale
+//     folded in, and a lazy rescale of O (only when the running max grows by more than 2^8);
+//   * block-causality is exploited at tile level: a Q-tile pair only visits the KV tiles its
+//     last row can see, and only boundary tiles pay for per-row column masking;
+//   * a persistent stream-K schedule splits the flattened (head, Q-pair, KV-tile) iteration space
+//     evenly over one CTA per SM; a segment that does not cover its whole KV range writes an
+//     FP32 partial (O, m, l) and a small combine kernel merges the partials.
+//
+// Roofline: tensor pipe.  Algorithmic flops = 4 * d * H * sum_b |block b| * kv_visible[b].
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cudaTypedefs.h>
+
+#include <cstring>
+#include <mutex>
+
+#include "ws_internal.h"
+#include "ws_ptx.cuh"
+
+namespace {
+
+constexpr int kBlockM = 128;  // query rows per tile (one TMEM lane each)
+constexpr int kBlockN = 128;  // keys per tile
+constexpr int kPairM = 2 * kBlockM;
+constexpr int kStages = 5;    // K/V ring slots
+constexpr int kThreads = 384; // warp 0 TMA, warp 1 MMA, warp 2 TMEM alloc, warp 3 idle, warps 4-7 / 8-11 softmax
+constexpr int kMaxPairs = 256;
+constexpr int kMaxCtas = 256; // upper bound on the persistent grid (workspace sizing)
+constexpr int kTmemCols = 512;
+constexpr float kLog2e = 1.4426950408889634f;
+constexpr float kLn2 = 0.6931471805599453f;
+constexpr float kRescaleThreshold = 8.0f;  // log2 units: P stays below 2^8
+
+struct alignas(64) Params {
+  CUtensorMap map_q, map_kn, map_vn, map_kc, map_vc;
+  void* out;
+  float* lse;
+  float* part_o;   // [slots][d/4][256][4]
+  float2* part_ml; // [slots][256] (m * scale * log2e, l)
+  int64_t cache_len;
+  int32_t Lq, H, Ln, n_blocks, n_pairs, n_cache_tiles;
+  float scale, scale_log2;
+  int32_t q_block_end[WS_MAX_MASK_BLOCKS];
+  int32_t kv_visible[WS_MAX_MASK_BLOCKS];
+};
+
+struct Sched {
+  int32_t pair_prefix[kMaxPairs + 1];  // KV-tile iterations before pair p (per head)
+};
+
+// ---------------------------------------------------------------------------------------------
+// schedule helpers (shared by the attention and the combine kernel)
+// ---------------------------------------------------------------------------------------------
+// The block tables are read straight from the __grid_constant__ parameter block (constant bank).
+__device__ __forceinline__ int block_of_row(const Params& p, int row) {
+  int lo = 0, hi = p.n_blocks - 1;  // first b with row < q_block_end[b]
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    if (row < p.q_block_end[mid]) hi = mid; else lo = mid + 1;
+  }
+  return lo;
+}
+
+__device__ __forceinline__ int tiles_for(const Params& p, int nvis) {
+  if (nvis <= 0) return 0;
+  if ((int64_t)nvis <= p.cache_len) return (nvis + kBlockN - 1) / kBlockN;
+  return p.n_cache_tiles + (int)((nvis - p.cache_len + kBlockN - 1) / kBlockN);
+}
+
+// All threads of the CTA call this; ends with __syncthreads().
+__device__ void build_sched(const Params& p, Sched& s) {
+  for (int pr = threadIdx.x; pr < p.n_pairs; pr += blockDim.x) {
+    const int last_row = min((pr + 1) * kPairM, p.Lq) - 1;
+    s.pair_prefix[pr + 1] = tiles_for(p, p.kv_visible[block_of_row(p, last_row)]);
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    s.pair_prefix[0] = 0;
+    for (int pr = 0; pr < p.n_pairs; ++pr) s.pair_prefix[pr + 1] += s.pair_prefix[pr];
+  }
+  __syncthreads();
+}
+
+__device__ __forceinline__ int pair_of_iter(const Sched& s, int n_pairs, int rem) {
+  int lo = 0, hi = n_pairs - 1;  // largest p with pair_prefix[p] <= rem
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if (s.pair_prefix[mid] <= rem) lo = mid; else hi = mid - 1;
+  }
+  return lo;
+}
+
+__device__ __forceinline__ int64_t cta_begin(int64_t c, int64_t T, int64_t G) { return (c * T) / G; }
+__device__ __forceinline__ int cta_of_iter(int64_t t, int64_t T, int64_t G) { return (int)(((t + 1) * G - 1) / T); }
+
+struct Segment {
+  int head, pair, j0, j1, n_tiles;  // KV tiles [j0, j1) of the pair's n_tiles
+};
+
+// Walks the CTA's share [t, hi) of the flattened iteration space.
+__device__ __forceinline__ Segment next_segment(const Sched& s, const Params& p, int64_t& t, int64_t hi) {
+  const int Tp = s.pair_prefix[p.n_pairs];
+  Segment g;
+  g.head = (int)(t / Tp);
+  const int rem = (int)(t - (int64_t)g.head * Tp);
+  g.pair = pair_of_iter(s, p.n_pairs, rem);
+  g.n_tiles = s.pair_prefix[g.pair + 1] - s.pair_prefix[g.pair];
+  g.j0 = rem - s.pair_prefix[g.pair];
+  const int64_t left = hi - t;
+  g.j1 = (int)min((int64_t)g.n_tiles, g.j0 + left);
+  t += g.j1 - g.j0;
+  return g;
+}
+
+// ---------------------------------------------------------------------------------------------
+// the attention kernel
+// ---------------------------------------------------------------------------------------------
+template <int D>
+struct Cfg {
+  static constexpr int kAtoms = D / 64;                   // 64-element (128-byte) swizzle atoms along d
+  static constexpr int kAtomBytes = kBlockN * 128;        // [128 rows][128 B]
+  static constexpr int kTileBytes = kAtoms * kAtomBytes;  // one Q tile == one K or V tile
+  static constexpr int kSmemQ = 2 * kTileBytes;
+  static constexpr int kSmemKV = kStages * kTileBytes;
+  static constexpr int kSmemBytes = 1024 /*align slack*/ + kSmemQ + kSmemKV + 256 /*barriers*/ + (int)sizeof(Sched);
+  static constexpr uint32_t kTmemS0 = 0, kTmemS1 = 128, kTmemO0 = 256, kTmemO1 = 256 + D;
+  static constexpr uint32_t kIdescQK = ptx::make_idesc_bf16(kBlockM, kBlockN, false);
+  static constexpr uint32_t kIdescPV = ptx::make_idesc_bf16(kBlockM, D, true);
+};
+
+struct Barriers {
+  uint64_t kv_full[kStages], kv_empty[kStages];
+  uint64_t q_full, q_empty;
+  uint64_t s_full[2], p_full[2], o_done[2];
+  uint32_t tmem_base;
+};
+
+template <int D, bool OUT_F32>
+__global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_constant__ Params p) {
+  using C = Cfg<D>;
+  extern __shared__ uint8_t smem_raw[];
+  // 1024-byte alignment is required by the 128-byte swizzle (TMA box and UMMA descriptor agree on it)
+  const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
+  uint8_t* smem = smem_raw + (smem_base - ptx::smem_u32(smem_raw));
+  const uint32_t sQ = smem_base;
+  const uint32_t sKV = smem_base + C::kSmemQ;
+  Barriers& bar = *reinterpret_cast<Barriers*>(smem + C::kSmemQ + C::kSmemKV);
+  Sched& sched = *reinterpret_cast<Sched*>(smem + C::kSmemQ + C::kSmemKV + 256);
+  static_assert(sizeof(Barriers) <= 256, "barrier block");
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < kStages; ++i) {
+      ptx::mbar_init(ptx::smem_u32(&bar.kv_full[i]), 1);
+      ptx::mbar_init(ptx::smem_u32(&bar.kv_empty[i]), 1);
+    }
+    ptx::mbar_init(ptx::smem_u32(&bar.q_full), 1);
+    ptx::mbar_init(ptx::smem_u32(&bar.q_empty), 1);
+    for (int t = 0; t < 2; ++t) {
+      ptx::mbar_init(ptx::smem_u32(&bar.s_full[t]), 1);
+      ptx::mbar_init(ptx::smem_u32(&bar.p_full[t]), kBlockM);
+      ptx::mbar_init(ptx::smem_u32(&bar.o_done[t]), 1);
+    }
+    ptx::fence_mbar_init();
+    ptx::prefetch_tensormap(&p.map_q);
+    ptx::prefetch_tensormap(&p.map_kc);
+    ptx::prefetch_tensormap(&p.map_vc);
+    ptx::prefetch_tensormap(&p.map_kn);
+    ptx::prefetch_tensormap(&p.map_vn);
+  }
+  if (warp == 2) {
+    ptx::tmem_alloc(ptx::smem_u32(&bar.tmem_base), kTmemCols);
+    ptx::tmem_relinquish();
+  }
+  build_sched(p, sched);  // includes __syncthreads()
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::tc_fence_after();
+  const uint32_t tmem = bar.tmem_base;
+
+  const int Tp = sched.pair_prefix[p.n_pairs];
+  const int64_t T = (int64_t)Tp * p.H;
+  const int64_t t_lo = cta_begin(blockIdx.x, T, gridDim.x), t_hi = cta_begin(blockIdx.x + 1, T, gridDim.x);
+
+  if (warp < 4) {
+    ptx::setmaxnreg_dec<56>();
+    if (warp == 0 && lane == 0) {
+      // ============================== TMA producer ==============================
+      uint32_t it = 0, seg = 0;
+      auto load_kv = [&](const Segment& g, int j, bool is_v) {
+        const uint32_t slot = it % kStages, ph = (it / kStages) & 1;
+        ptx::mbar_wait(ptx::smem_u32(&bar.kv_empty[slot]), ph ^ 1);
+        const uint32_t full = ptx::smem_u32(&bar.kv_full[slot]);
+        ptx::mbar_arrive_expect_tx(full, C::kTileBytes);
+        const uint32_t dst = sKV + slot * C::kTileBytes;
+        if (j < p.n_cache_tiles) {
+          const void* map = is_v ? (const void*)&p.map_vc : (const void*)&p.map_kc;
+#pragma unroll
+          for (int a = 0; a < C::kAtoms; ++a) ptx::tma_load_3d(dst + a * C::kAtomBytes, map, full, a * 64, j * kBlockN, g.head);
+        } else {
+          const void* map = is_v ? (const void*)&p.map_vn : (const void*)&p.map_kn;
+          const int r0 = (j - p.n_cache_tiles) * kBlockN;
+#pragma unroll
+          for (int a = 0; a < C::kAtoms; ++a) ptx::tma_load_3d(dst + a * C::kAtomBytes, map, full, a * 64, g.head, r0);
+        }
+        ++it;
+      };
+      for (int64_t t = t_lo; t < t_hi; ++seg) {
+        const Segment g = next_segment(sched, p, t, t_hi);
+        ptx::mbar_wait(ptx::smem_u32(&bar.q_empty), (seg & 1) ^ 1);
+        const uint32_t qf = ptx::smem_u32(&bar.q_full);
+        ptx::mbar_arrive_expect_tx(qf, 2 * C::kTileBytes);
+#pragma unroll
+        for (int tile = 0; tile < 2; ++tile)
+#pragma unroll
+          for (int a = 0; a < C::kAtoms; ++a)
+            ptx::tma_load_3d(sQ + tile * C::kTileBytes + a * C::kAtomBytes, &p.map_q, qf, a * 64, g.head,
+                             g.pair * kPairM + tile * kBlockM);
+        load_kv(g, g.j0, false);
+        for (int j = g.j0; j < g.j1; ++j) {
+          load_kv(g, j, true);
+          if (j + 1 < g.j1) load_kv(g, j + 1, false);
+        }
+      }
+    } else if (warp == 1 && lane == 0) {
+      // ============================== MMA issuer ==============================
+      uint32_t it = 0, seg = 0, p_phase = 0;
+      const uint32_t tS[2] = {tmem + C::kTmemS0, tmem + C::kTmemS1};
+      const uint32_t tO[2] = {tmem + C::kTmemO0, tmem + C::kTmemO1};
+      auto issue_qk = [&](int tile, uint32_t slot) {
+        const uint32_t qa = sQ + tile * C::kTileBytes, kb = sKV + slot * C::kTileBytes;
+#pragma unroll
+        for (int k = 0; k < D / 16; ++k) {
+          const uint32_t off = (k >> 2) * C::kAtomBytes + (k & 3) * 32;
+          ptx::mma_ss(tS[tile], ptx::make_sdesc_sw128(qa + off, 16, 1024), ptx::make_sdesc_sw128(kb + off, 16, 1024),
+                      C::kIdescQK, k > 0);
+        }
+      };
+      auto issue_pv = [&](int tile, uint32_t slot, bool acc) {
+        const uint32_t vb = sKV + slot * C::kTileBytes;
+#pragma unroll
+        for (int k = 0; k < kBlockN / 16; ++k)
+          ptx::mma_ts(tO[tile], tS[tile] + k * 8, ptx::make_sdesc_sw128(vb + k * 2048, C::kAtomBytes, 1024), C::kIdescPV,
+                      acc || k > 0);
+      };
+      auto wait_full = [&](uint32_t i) {
+        ptx::mbar_wait(ptx::smem_u32(&bar.kv_full[i % kStages]), (i / kStages) & 1);
+        ptx::tc_fence_after();
+      };
+      for (int64_t t = t_lo; t < t_hi; ++seg) {
+        const Segment g = next_segment(sched, p, t, t_hi);
+        ptx::mbar_wait(ptx::smem_u32(&bar.q_full), seg & 1);
+        wait_full(it);
+        {
+          const uint32_t slot = it % kStages;
+          issue_qk(0, slot);
+          ptx::tc_commit(ptx::smem_u32(&bar.s_full[0]));
+          issue_qk(1, slot);
+          ptx::tc_commit(ptx::smem_u32(&bar.s_full[1]));
+          ptx::tc_commit(ptx::smem_u32(&bar.kv_empty[slot]));
+          if (g.j0 + 1 == g.j1) ptx::tc_commit(ptx::smem_u32(&bar.q_empty));
+          ++it;
+        }
+        for (int j = g.j0; j < g.j1; ++j) {
+          const bool has_next = j + 1 < g.j1, acc = j > g.j0;
+          const uint32_t it_v = it++, slot_v = it_v % kStages;
+          uint32_t it_k = 0, slot_k = 0;
+          if (has_next) { it_k = it++; slot_k = it_k % kStages; }
+          wait_full(it_v);
+          ptx::mbar_wait(ptx::smem_u32(&bar.p_full[0]), p_phase);
+          ptx::tc_fence_after();
+          issue_pv(0, slot_v, acc);
+          ptx::tc_commit(ptx::smem_u32(&bar.o_done[0]));
+          if (has_next) {
+            wait_full(it_k);
+            issue_qk(0, slot_k);
+            ptx::tc_commit(ptx::smem_u32(&bar.s_full[0]));
+          }
+          ptx::mbar_wait(ptx::smem_u32(&bar.p_full[1]), p_phase);
+          ptx::tc_fence_after();
+          issue_pv(1, slot_v, acc);
+          ptx::tc_commit(ptx::smem_u32(&bar.o_done[1]));
+          ptx::tc_commit(ptx::smem_u32(&bar.kv_empty[slot_v]));
+          if (has_next) {
+            issue_qk(1, slot_k);
+            ptx::tc_commit(ptx::smem_u32(&bar.s_full[1]));
+            ptx::tc_commit(ptx::smem_u32(&bar.kv_empty[slot_k]));
+            if (j + 2 == g.j1) ptx::tc_commit(ptx::smem_u32(&bar.q_empty));
+          }
+          p_phase ^= 1;
+        }
+      }
+    }
+  } else {
+    // ============================== softmax warpgroups ==============================
+    ptx::setmaxnreg_inc<224>();
+    const int tile = (warp - 4) >> 2;                    // 0 or 1: which Q tile of the pair
+    const int row_in_tile = ((warp & 3) << 5) | lane;    // == TMEM lane this thread may access
+    const uint32_t lane_off = (uint32_t)((warp & 3) << 5) << 16;
+    const uint32_t tS = tmem + (tile ? C::kTmemS1 : C::kTmemS0) + lane_off;
+    const uint32_t tO = tmem + (tile ? C::kTmemO1 : C::kTmemO0) + lane_off;
+    const uint32_t s_full = ptx::smem_u32(&bar.s_full[tile]), p_full = ptx::smem_u32(&bar.p_full[tile]);
+    const uint32_t o_done = ptx::smem_u32(&bar.o_done[tile]);
+    uint32_t n_iter = 0;  // S tiles consumed so far == PVs requested so far (drives every phase bit)
+
+    for (int64_t t = t_lo; t < t_hi;) {
+      const Segment g = next_segment(sched, p, t, t_hi);
+      const int row = g.pair * kPairM + tile * kBlockM + row_in_tile;
+      const bool row_valid = row < p.Lq;
+      const int nvis = row_valid ? p.kv_visible[block_of_row(p, row)] : 0;
+      const int vis_cache = (int)min((int64_t)nvis, p.cache_len);
+      float m = -INFINITY, l = 0.f;  // running max in raw-score units, running sum
+
+      for (int j = g.j0; j < g.j1; ++j, ++n_iter) {
+        int lim;  // columns [0, lim) of this tile are visible to this row
+        if (j < p.n_cache_tiles) lim = vis_cache - j * kBlockN;
+        else lim = nvis - (int)p.cache_len - (j - p.n_cache_tiles) * kBlockN;
+
+        ptx::mbar_wait(s_full, n_iter & 1);
+        ptx::tc_fence_after();
+        uint32_t s[4][32];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) ptx::tmem_ld32(tS + q * 32, s[q]);
+        ptx::tc_wait_ld();
+        if (lim < kBlockN) {
+#pragma unroll
+          for (int q = 0; q < 4; ++q)
+#pragma unroll
+            for (int c = 0; c < 32; ++c)
+              if (q * 32 + c >= lim) s[q][c] = 0xff800000u;  // -inf
+        }
+        float mx = __uint_as_float(s[0][0]);
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+#pragma unroll
+          for (int c = 0; c < 32; ++c) mx = fmaxf(mx, __uint_as_float(s[q][c]));
+        const float m_new = fmaxf(m, mx);
+        const bool grow = (m_new - m) * p.scale_log2 > kRescaleThreshold;  // false when both are -inf (NaN)
+        if (j == g.j0) {
+          m = m_new;  // O is overwritten by the first P.V of the segment: nothing to rescale
+        } else if (__any_sync(0xffffffffu, grow)) {
+          // lazy rescale of the accumulator in TMEM: needs the previous P.V to have landed
+          ptx::mbar_wait(o_done, (n_iter - 1) & 1);
+          ptx::tc_fence_after();
+          const float f = grow ? ptx::ex2((m - m_new) * p.scale_log2) : 1.f;
+          if (grow) { m = m_new; l *= f; }
+#pragma unroll
+          for (int ch = 0; ch < D / 32; ++ch) {
+            uint32_t o[32];
+            ptx::tmem_ld32(tO + ch * 32, o);
+            ptx::tc_wait_ld();
+#pragma unroll
+            for (int c = 0; c < 32; ++c) o[c] = __float_as_uint(__uint_as_float(o[c]) * f);
+            ptx::tmem_st32(tO + ch * 32, o);
+          }
+        }
+        const float neg_ms = (m == -INFINITY) ? 0.f : -m * p.scale_log2;
+        uint32_t pk[2][32];
+        float sum0 = 0.f, sum1 = 0.f;
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+#pragma unroll
+          for (int c = 0; c < 32; c += 2) {
+            const float p0 = ptx::ex2(fmaf(__uint_as_float(s[q][c]), p.scale_log2, neg_ms));
+            const float p1 = ptx::ex2(fmaf(__uint_as_float(s[q][c + 1]), p.scale_log2, neg_ms));
+            sum0 += p0;
+            sum1 += p1;
+            pk[q >> 1][((q & 1) << 4) | (c >> 1)] = ptx::pack_bf16(p0, p1);
+          }
+        l += sum0 + sum1;
+        ptx::tmem_st32(tS, pk[0]);
+        ptx::tmem_st32(tS + 32, pk[1]);
+        ptx::tc_wait_st();
+        ptx::tc_fence_before();
+        ptx::mbar_arrive(p_full);
+      }
+
+      // ------------------------------ segment epilogue ------------------------------
+      ptx::mbar_wait(o_done, (n_iter - 1) & 1);
+      ptx::tc_fence_after();
+      const bool whole = (g.j0 == 0 && g.j1 == g.n_tiles);
+      if (whole) {
+        const float inv = l > 0.f ? 1.f / l : 0.f;
+        if (p.lse != nullptr && row_valid)
+          p.lse[(int64_t)g.head * p.Lq + row] = l > 0.f ? (ptx::lg2(l) + m * p.scale_log2) * kLn2 : -INFINITY;
+#pragma unroll
+        for (int ch = 0; ch < D / 32; ++ch) {
+          uint32_t o[32];
+          ptx::tmem_ld32(tO + ch * 32, o);
+          ptx::tc_wait_ld();
+          if (row_valid) {
+            if constexpr (OUT_F32) {
+              float4* dst = reinterpret_cast<float4*>(reinterpret_cast<float*>(p.out) + ((int64_t)row * p.H + g.head) * D + ch * 32);
+#pragma unroll
+              for (int c = 0; c < 8; ++c)
+                dst[c] = make_float4(__uint_as_float(o[4 * c]) * inv, __uint_as_float(o[4 * c + 1]) * inv,
+                                     __uint_as_float(o[4 * c + 2]) * inv, __uint_as_float(o[4 * c + 3]) * inv);
+            } else {
+              uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<__nv_bfloat16*>(p.out) + ((int64_t)row * p.H + g.head) * D + ch * 32);
+#pragma unroll
+              for (int c = 0; c < 4; ++c) {
+                uint4 v;
+                v.x = ptx::pack_bf16(__uint_as_float(o[8 * c]) * inv, __uint_as_float(o[8 * c + 1]) * inv);
+                v.y = ptx::pack_bf16(__uint_as_float(o[8 * c + 2]) * inv, __uint_as_float(o[8 * c + 3]) * inv);
+                v.z = ptx::pack_bf16(__uint_as_float(o[8 * c + 4]) * inv, __uint_as_float(o[8 * c + 5]) * inv);
+                v.w = ptx::pack_bf16(__uint_as_float(o[8 * c + 6]) * inv, __uint_as_float(o[8 * c + 7]) * inv);
+                dst[c] = v;
+              }
+            }
+          }
+        }
+      } else {
+        // partial: unnormalised O (FP32), running max (log2 units) and sum, into slot work + cta
+        const int64_t slot = (int64_t)g.head * p.n_pairs + g.pair + blockIdx.x;
+        const int r = tile * kBlockM + row_in_tile;
+        p.part_ml[slot * kPairM + r] = make_float2(m == -INFINITY ? -INFINITY : m * p.scale_log2, l);
+        float4* po = reinterpret_cast<float4*>(p.part_o) + slot * (D / 4) * kPairM + r;
+#pragma unroll
+        for (int ch = 0; ch < D / 32; ++ch) {
+          uint32_t o[32];
+          ptx::tmem_ld32(tO + ch * 32, o);
+          ptx::tc_wait_ld();
+#pragma unroll
+          for (int c = 0; c < 8; ++c)
+            po[(int64_t)(ch * 8 + c) * kPairM] = make_float4(__uint_as_float(o[4 * c]), __uint_as_float(o[4 * c + 1]),
+                                                             __uint_as_float(o[4 * c + 2]), __uint_as_float(o[4 * c + 3]));
+        }
+      }
+      // the next segment's first P.V overwrites O: order our TMEM reads before the p_full arrive that unleashes it
+      ptx::tc_fence_before();
+    }
+  }
+
+  ptx::tc_fence_before();
+  __syncthreads();
+  if (warp == 2) ptx::tmem_dealloc(tmem, kTmemCols);
+}
+
+// ---------------------------------------------------------------------------------------------
+// combine kernel: merges split-KV partials, and zero-fills Q-pairs that see no key at all.
+// grid = (d/4, H * n_pairs), block = 256 threads (one per row of the pair).
+// ---------------------------------------------------------------------------------------------
+template <int D, bool OUT_F32>
+__global__ void __launch_bounds__(kPairM) attn_combine_kernel(const __grid_constant__ Params p, int attn_grid) {
+  __shared__ Sched sched;
+  build_sched(p, sched);
+  const int w = blockIdx.y, head = w / p.n_pairs, pair = w - head * p.n_pairs;
+  const int q4 = blockIdx.x, r = threadIdx.x;
+  const int row = pair * kPairM + r;
+  if (row >= p.Lq) return;
+  const int Tp = sched.pair_prefix[p.n_pairs];
+  const int n_tiles = sched.pair_prefix[pair + 1] - sched.pair_prefix[pair];
+  float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+  float lse = -INFINITY;
+  if (n_tiles > 0) {
+    const int64_t T = (int64_t)Tp * p.H;
+    const int64_t a = (int64_t)head * Tp + sched.pair_prefix[pair];
+    const int c_lo = cta_of_iter(a, T, attn_grid), c_hi = cta_of_iter(a + n_tiles - 1, T, attn_grid);
+    if (c_lo == c_hi) return;  // one CTA covered the whole KV range and wrote the final rows itself
+    float M = -INFINITY;
+    for (int c = c_lo; c <= c_hi; ++c) M = fmaxf(M, p.part_ml[((int64_t)w + c) * kPairM + r].x);
+    float L = 0.f;
+    if (M > -INFINITY) {
+      for (int c = c_lo; c <= c_hi; ++c) {
+        const int64_t slot = (int64_t)w + c;
+        const float2 ml = p.part_ml[slot * kPairM + r];
+        const float wgt = ptx::ex2(ml.x - M);  // 0 for an all-masked partial (m = -inf)
+        const float4 o = reinterpret_cast<const float4*>(p.part_o)[(slot * (D / 4) + q4) * kPairM + r];
+        acc.x += wgt * o.x; acc.y += wgt * o.y; acc.z += wgt * o.z; acc.w += wgt * o.w;
+        L += wgt * ml.y;
+      }
+    }
+    if (L > 0.f) {
+      const float inv = 1.f / L;
+      acc.x *= inv; acc.y *= inv; acc.z *= inv; acc.w *= inv;
+      lse = (ptx::lg2(L) + M) * kLn2;
+    } else {
+      acc = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+  }
+  const int64_t o_off = ((int64_t)row * p.H + head) * D + q4 * 4;
+  if constexpr (OUT_F32) {
+    *reinterpret_cast<float4*>(reinterpret_cast<float*>(p.out) + o_off) = acc;
+  } else {
+    uint2 v;
+    v.x = ptx::pack_bf16(acc.x, acc.y);
+    v.y = ptx::pack_bf16(acc.z, acc.w);
+    *reinterpret_cast<uint2*>(reinterpret_cast<__nv_bfloat16*>(p.out) + o_off) = v;
+  }
+  if (q4 == 0 && p.lse != nullptr) p.lse[(int64_t)head * p.Lq + row] = lse;
+}
+
+// FP32 -> BF16 staging for WS_DTYPE_F32 inputs (config 1; R9).
+// Copies `rows` rows of `row_elems` contiguous floats; source rows `src_pitch` floats apart per plane.
+__global__ void cast_f32_to_bf16_kernel(__nv_bfloat16* __restrict__ dst, const float* __restrict__ src, int64_t n_planes,
+                                        int64_t plane_elems, int64_t src_plane_pitch) {
+  const int64_t total = n_planes * plane_elems;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t pl = i / plane_elems, e = i - pl * plane_elems;
+    dst[i] = __float2bfloat16_rn(src[pl * src_plane_pitch + e]);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------------------
+PFN_cuTensorMapEncodeTiled_v12000 get_encode_fn() {
+  static PFN_cuTensorMapEncodeTiled_v12000 fn = nullptr;
+  static std::once_flag once;
+  std::call_once(once, [] {
+    void* f = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(f);
+  });
+  return fn;
+}
+
+// 3-D BF16 tensor map, 128-byte swizzle, box = {64 elements, b1, b2}.
+bool encode_map(CUtensorMap* map, const void* base, uint64_t d0, uint64_t d1, uint64_t d2, uint64_t stride1_bytes,
+                uint64_t stride2_bytes, uint32_t b1, uint32_t b2) {
+  auto fn = get_encode_fn();
+  if (!fn) return false;
+  cuuint64_t dims[3] = {d0, d1, d2};
+  cuuint64_t strides[2] = {stride1_bytes, stride2_bytes};
+  cuuint32_t box[3] = {64, b1, b2};
+  cuuint32_t estr[3] = {1, 1, 1};
+  return fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+int sm_count() {
+  static int n = 0;
+  if (n == 0) {
+    int dev = 0, v = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess)
+      n = v;
+  }
+  return n;
+}
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct WsLayout {
+  size_t part_o, part_ml, stage_q, stage_kc, stage_vc, stage_kn, stage_vn, total;
+};
+
+WsLayout ws_layout(int32_t Lq, int32_t H, int32_t d, int64_t kv_total, int64_t cache_len, int32_t Ln, ws_dtype dt,
+                   bool exact) {
+  WsLayout L{};
+  const size_t n_pairs = (size_t)(Lq + kPairM - 1) / kPairM;
+  const size_t slots = n_pairs * H + kMaxCtas;
+  size_t off = 0;
+  L.part_o = off; off = align_up(off + slots * kPairM * (size_t)d * 4, 256);
+  L.part_ml = off; off = align_up(off + slots * kPairM * 8, 256);
+  if (dt == WS_DTYPE_F32) {
+    L.stage_q = off; off = align_up(off + (size_t)Lq * H * d * 2, 256);
+    if (exact) {
+      L.stage_kc = off; off = align_up(off + (size_t)H * cache_len * d * 2, 256);
+      L.stage_vc = off; off = align_up(off + (size_t)H * cache_len * d * 2, 256);
+      L.stage_kn = off; off = align_up(off + (size_t)Ln * H * d * 2, 256);
+      L.stage_vn = off; off = align_up(off + (size_t)Ln * H * d * 2, 256);
+    } else {  // size query: only cache_len + Ln is known; each of the four regions may need its own rounding
+      off = align_up(off + 2 * (size_t)H * kv_total * d * 2, 256) + 4 * 256;
+    }
+  }
+  L.total = off;
+  return L;
+}
+
+template <int D, bool OUT_F32>
+int launch_attention(const Params& prm, int64_t total_iters, cudaStream_t stream) {
+  using C = Cfg<D>;
+  static std::once_flag once;
+  static cudaError_t attr_err = cudaSuccess;
+  std::call_once(once, [] {
+    attr_err = cudaFuncSetAttribute(attn_fwd_kernel<D, OUT_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes);
+  });
+  if (attr_err != cudaSuccess) return wsi::cuda_fail(attr_err);
+  const int sms = sm_count();
+  if (sms <= 0) return wsi::cuda_fail(cudaErrorNoDevice);
+  int grid = (int)(total_iters < (int64_t)sms ? total_iters : (int64_t)sms);
+  if (grid > kMaxCtas) grid = kMaxCtas;
+  int launches = 0;
+  if (grid > 0) {
+    attn_fwd_kernel<D, OUT_F32><<<grid, kThreads, C::kSmemBytes, stream>>>(prm);
+    ++launches;
+  }
+  dim3 cgrid(D / 4, (unsigned)(prm.H * prm.n_pairs));
+  attn_combine_kernel<D, OUT_F32><<<cgrid, kPairM, 0, stream>>>(prm, grid > 0 ? grid : 1);
+  ++launches;
+  return wsi::after_launch(launches);
+}
+
+}  // namespace
+
+extern "C" __attribute__((visibility("default"))) size_t ws_block_causal_attn_workspace_bytes(int32_t Lq, int32_t H, int32_t d, int64_t kv_total, ws_dtype dt) {
+  if (Lq <= 0 || H <= 0 || d <= 0 || kv_total < 0) return 0;
+  return ws_layout(Lq, H, d, kv_total, 0, 0, dt, false).total;
+}
+
+extern "C" __attribute__((visibility("default"))) int ws_block_causal_attn(void* out, float* lse, const void* q, const void* k_cache, const void* v_cache,
+                                    int64_t capacity, int64_t cache_len, const void* k_new, const void* v_new, int32_t Ln,
+                                    int32_t H, int32_t d, int32_t Lq, const ws_block_mask* mask, float softmax_scale,
+                                    void* workspace, size_t workspace_bytes, ws_dtype dt, void* stream_) {
+  cudaStream_t stream = (cudaStream_t)stream_;
+  // ---- validation: nothing is launched on any error ----
+  if (dt != WS_DTYPE_BF16 && dt != WS_DTYPE_F32) return WS_ERR_UNSUPPORTED;
+  if (d != 64 && d != 128) return WS_ERR_UNSUPPORTED;
+  if (!out || !q || !mask || H <= 0 || Lq <= 0 || Ln < 0 || capacity < 0 || cache_len < 0) return WS_ERR_INVALID_ARG;
+  if (!(softmax_scale >= 0.f) || !(softmax_scale < INFINITY)) return WS_ERR_INVALID_ARG;
+  if ((Ln > 0) != (k_new != nullptr) || (Ln > 0) != (v_new != nullptr)) return WS_ERR_INVALID_ARG;
+  if (cache_len > capacity) return WS_ERR_OUT_OF_RANGE;
+  if (cache_len > 0 && (!k_cache || !v_cache)) return WS_ERR_INVALID_ARG;
+  if (mask->n_blocks <= 0 || !mask->q_block_end || !mask->kv_visible) return WS_ERR_INVALID_ARG;
+  if (mask->n_blocks > WS_MAX_MASK_BLOCKS) return WS_ERR_UNSUPPORTED;
+  if (cache_len + Ln > 0x7fffffffLL - kBlockN) return WS_ERR_UNSUPPORTED;
+  {
+    int32_t prev_end = 0, prev_vis = 0;
+    for (int b = 0; b < mask->n_blocks; ++b) {
+      if (mask->q_block_end[b] <= prev_end || mask->kv_visible[b] < prev_vis) return WS_ERR_INVALID_ARG;
+      if ((int64_t)mask->kv_visible[b] > cache_len + Ln) return WS_ERR_OUT_OF_RANGE;
+      prev_end = mask->q_block_end[b];
+      prev_vis = mask->kv_visible[b];
+    }
+    if (prev_end != Lq) return WS_ERR_INVALID_ARG;
+  }
+  const int n_pairs = (Lq + kPairM - 1) / kPairM;
+  if (n_pairs > kMaxPairs) return WS_ERR_UNSUPPORTED;
+  if (!wsi::aligned16(out) || !wsi::aligned16(q) || !wsi::aligned16(k_cache) || !wsi::aligned16(v_cache) ||
+      !wsi::aligned16(k_new) || !wsi::aligned16(v_new) || (lse && (reinterpret_cast<uintptr_t>(lse) & 3)))
+    return WS_ERR_ALIGNMENT;
+  const WsLayout L = ws_layout(Lq, H, d, cache_len + Ln, cache_len, Ln, dt, true);
+  if (!workspace || workspace_bytes < L.total) return WS_ERR_WORKSPACE;
+  if (!wsi::aligned256(workspace)) return WS_ERR_WORKSPACE;
+  if (!get_encode_fn()) return wsi::cuda_fail(cudaErrorNotSupported);
+
+  char* ws = reinterpret_cast<char*>(workspace);
+  const void *q_b = q, *kc_b = k_cache, *vc_b = v_cache, *kn_b = k_new, *vn_b = v_new;
+  int64_t cap_b = capacity;
+  int launches = 0;
+  if (dt == WS_DTYPE_F32) {
+    // round the FP32 operands to BF16 on the device (reading R9); the cache copy is compacted to cache_len rows
+    auto cast = [&](void* dstp, const void* srcp, int64_t planes, int64_t plane_elems, int64_t pitch) {
+      const int64_t total = planes * plane_elems;
+      if (total == 0) return;
+      const int blocks = (int)((total + 255) / 256 < 4096 ? (total + 255) / 256 : 4096);
+      cast_f32_to_bf16_kernel<<<blocks, 256, 0, stream>>>(reinterpret_cast<__nv_bfloat16*>(dstp),
+                                                          reinterpret_cast<const float*>(srcp), planes, plane_elems, pitch);
+      ++launches;
+    };
+    cast(ws + L.stage_q, q, 1, (int64_t)Lq * H * d, 0);
+    cast(ws + L.stage_kc, k_cache, H, cache_len * d, capacity * d);
+    cast(ws + L.stage_vc, v_cache, H, cache_len * d, capacity * d);
+    cast(ws + L.stage_kn, k_new, 1, (int64_t)Ln * H * d, 0);
+    cast(ws + L.stage_vn, v_new, 1, (int64_t)Ln * H * d, 0);
+    q_b = ws + L.stage_q; kc_b = ws + L.stage_kc; vc_b = ws + L.stage_vc; kn_b = ws + L.stage_kn; vn_b = ws + L.stage_vn;
+    cap_b = cache_len;
+  }
+
+  Params prm;
+  memset(&prm, 0, sizeof(prm));
+  const uint64_t row_b = (uint64_t)d * 2;
+  bool ok = encode_map(&prm.map_q, q_b, d, H, Lq, row_b, row_b * H, 1, kBlockM);
+  // a source with no rows still needs a well-formed (never dereferenced) descriptor
+  ok = ok && (Ln > 0 ? encode_map(&prm.map_kn, kn_b, d, H, Ln, row_b, row_b * H, 1, kBlockN)
+                     : encode_map(&prm.map_kn, q_b, d, H, Lq, row_b, row_b * H, 1, kBlockN));
+  ok = ok && (Ln > 0 ? encode_map(&prm.map_vn, vn_b, d, H, Ln, row_b, row_b * H, 1, kBlockN)
+                     : encode_map(&prm.map_vn, q_b, d, H, Lq, row_b, row_b * H, 1, kBlockN));
+  ok = ok && (cache_len > 0 ? encode_map(&prm.map_kc, kc_b, d, cache_len, H, row_b, row_b * cap_b, kBlockN, 1)
+                            : encode_map(&prm.map_kc, q_b, d, H, Lq, row_b, row_b * H, 1, kBlockN));
+  ok = ok && (cache_len > 0 ? encode_map(&prm.map_vc, vc_b, d, cache_len, H, row_b, row_b * cap_b, kBlockN, 1)
+                            : encode_map(&prm.map_vc, q_b, d, H, Lq, row_b, row_b * H, 1, kBlockN));
+  if (!ok) return wsi::cuda_fail(cudaErrorInvalidValue);
+  prm.out = out;
+  prm.lse = lse;
+  prm.part_o = reinterpret_cast<float*>(ws + L.part_o);
+  prm.part_ml = reinterpret_cast<float2*>(ws + L.part_ml);
+  prm.cache_len = cache_len;
+  prm.Lq = Lq; prm.H = H; prm.Ln = Ln; prm.n_blocks = mask->n_blocks; prm.n_pairs = n_pairs;
+  prm.n_cache_tiles = (int)((cache_len + kBlockN - 1) / kBlockN);
+  prm.scale = softmax_scale;
+  // clamped away from 0 so that a masked (-inf) logit times the scale stays -inf (softmax_scale == 0 is legal)
+  prm.scale_log2 = fmaxf(softmax_scale * kLog2e, 1e-30f);
+  for (int b = 0; b < mask->n_blocks; ++b) {
+    prm.q_block_end[b] = mask->q_block_end[b];
+    prm.kv_visible[b] = mask->kv_visible[b];
+  }
+  // total KV-tile iterations (host copy of the device schedule)
+  int64_t Tp = 0;
+  for (int pr = 0; pr < n_pairs; ++pr) {
+    const int last_row = ((pr + 1) * kPairM < Lq ? (pr + 1) * kPairM : Lq) - 1;
+    int b = 0;
+    while (last_row >= mask->q_block_end[b]) ++b;
+    const int64_t nvis = mask->kv_visible[b];
+    if (nvis <= 0) continue;
+    Tp += nvis <= cache_len ? (nvis + kBlockN - 1) / kBlockN : prm.n_cache_tiles + (nvis - cache_len + kBlockN - 1) / kBlockN;
+  }
+  if (launches) wsi::count_launch(launches);
+  const bool f32 = dt == WS_DTYPE_F32;
+  if (d == 128) return f32 ? launch_attention<128, true>(prm, Tp * H, stream) : launch_attention<128, false>(prm, Tp * H, stream);
+  return f32 ? launch_attention<64, true>(prm, Tp * H, stream) : launch_attention<64, false>(prm, Tp * H, stream);
+}

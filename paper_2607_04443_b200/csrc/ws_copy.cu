@@ -1,0 +1,150 @@
+// ws_copy.cu -- the three HBM-bound byte movers of the hot path, one kernel.
+//
+//   ws_kv_cache_write  slice [n, H_src, d]  -> cache [H, capacity, d]
+//   ws_seq_to_head       [n_tok, H, d]        -> [G, n_tok, H/P, d]
+//   ws_head_to_seq       inverse
+//
+// All three are "copy A x B chunks of dv 16-byte vectors, with independent (a, b) strides on the
+// two sides".  Roofline: HBM; algorithmic bytes = payload read once + written once.  The kernel
+// keeps 8 independent 16-byte loads in flight per thread (128 B/thread, 32 KB/CTA), reads with
+// ld.global.nc.L1::no_allocate (streamed once) and writes with plain st.global so the freshly
+// written cache rows / relaid tensors stay in the 126 MB L2 for the attention kernel that follows.
+#include "ws_internal.h"
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kUnroll = 8;  // 16-byte vectors per thread
+
+struct CopyPlan {
+  uint32_t dv;     // 16-byte vectors per contiguous chunk
+  uint32_t per_a;  // B * dv: vectors per outer index a
+  int64_t src_a, src_b, dst_a, dst_b;  // strides in 16-byte vectors
+};
+
+__device__ __forceinline__ uint4 ld_stream(const uint4* p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+               : "l"(p));
+  return r;
+}
+
+// grid = (ceil(per_a / (kThreads*kUnroll)), A, n_tensors)
+__global__ void __launch_bounds__(kThreads) strided_copy16_kernel(const uint4* __restrict__ src0, uint4* __restrict__ dst0,
+                                                                  const uint4* __restrict__ src1, uint4* __restrict__ dst1,
+                                                                  CopyPlan p) {
+  const uint4* __restrict__ src = blockIdx.z == 0 ? src0 : src1;
+  uint4* __restrict__ dst = blockIdx.z == 0 ? dst0 : dst1;
+  const int64_t a = blockIdx.y;
+  src += a * p.src_a;
+  dst += a * p.dst_a;
+  const uint32_t base = blockIdx.x * (kThreads * kUnroll) + threadIdx.x;
+  uint4 v[kUnroll];
+  int64_t doff[kUnroll];
+#pragma unroll
+  for (int u = 0; u < kUnroll; ++u) {
+    const uint32_t idx = base + u * kThreads;
+    doff[u] = -1;
+    if (idx < p.per_a) {
+      const uint32_t b = idx / p.dv;
+      const uint32_t c = idx - b * p.dv;
+      v[u] = ld_stream(src + (int64_t)b * p.src_b + c);
+      doff[u] = (int64_t)b * p.dst_b + c;
+    }
+  }
+#pragma unroll
+  for (int u = 0; u < kUnroll; ++u)
+    if (doff[u] >= 0) dst[doff[u]] = v[u];
+}
+
+// Launches the plan, splitting B so that per_a stays below 2^30 vectors.
+int launch_copy(const void* s0, void* d0, const void* s1, void* d1, int n_tensors, int64_t A, int64_t B, int64_t dv,
+                int64_t src_a, int64_t src_b, int64_t dst_a, int64_t dst_b, cudaStream_t stream) {
+  if (A == 0 || B == 0 || dv == 0) return WS_OK;
+  if (A > 65535 || dv > (1 << 20)) return WS_ERR_UNSUPPORTED;
+  const int64_t max_b = ((int64_t)1 << 30) / dv;
+  int launches = 0;
+  for (int64_t b0 = 0; b0 < B; b0 += max_b) {
+    const int64_t nb = (B - b0 < max_b) ? (B - b0) : max_b;
+    CopyPlan p;
+    p.dv = (uint32_t)dv;
+    p.per_a = (uint32_t)(nb * dv);
+    p.src_a = src_a; p.src_b = src_b; p.dst_a = dst_a; p.dst_b = dst_b;
+    const uint4* ps0 = reinterpret_cast<const uint4*>(s0) + b0 * src_b;
+    uint4* pd0 = reinterpret_cast<uint4*>(d0) + b0 * dst_b;
+    const uint4* ps1 = s1 ? reinterpret_cast<const uint4*>(s1) + b0 * src_b : nullptr;
+    uint4* pd1 = d1 ? reinterpret_cast<uint4*>(d1) + b0 * dst_b : nullptr;
+    dim3 grid((unsigned)((p.per_a + kThreads * kUnroll - 1) / (kThreads * kUnroll)), (unsigned)A, (unsigned)n_tensors);
+    strided_copy16_kernel<<<grid, kThreads, 0, stream>>>(ps0, pd0, ps1, pd1, p);
+    ++launches;
+  }
+  return wsi::after_launch(launches);
+}
+
+int relayout(void* dst, const void* src, int64_t n_tok, int32_t H, int32_t d, int32_t P, int32_t g0, int32_t G, ws_dtype dt,
+             void* stream, bool to_head) {
+  const int es = wsi::elem_bytes(dt);
+  if (es == 0) return WS_ERR_UNSUPPORTED;
+  if (!dst || !src || n_tok < 0 || H <= 0 || d <= 0 || P <= 0 || H % P != 0 || g0 < 0 || G < 0 || g0 + G > P)
+    return WS_ERR_INVALID_ARG;
+  const int32_t Hp = H / P;
+  const int64_t chunk_bytes = (int64_t)Hp * d * es;  // contiguous bytes per (g, t)
+  if (!wsi::aligned16(dst) || !wsi::aligned16(src) || ((int64_t)d * es) % 16 != 0) return WS_ERR_ALIGNMENT;
+  const size_t tok_bytes = (size_t)n_tok * H * d * es;          // token-major tensor
+  const size_t head_bytes = (size_t)G * n_tok * chunk_bytes;    // head-major tensor
+  if (wsi::ranges_overlap(dst, to_head ? head_bytes : tok_bytes, src, to_head ? tok_bytes : head_bytes)) return WS_ERR_OVERLAP;
+  const int64_t dv = chunk_bytes / 16;
+  const int64_t tok_a = (int64_t)Hp * d * es / 16;   // token-major: group g -> + g * Hp heads
+  const int64_t tok_b = (int64_t)H * d * es / 16;    // token t
+  const int64_t head_a = n_tok * dv;                 // head-major: group g
+  const int64_t head_b = dv;                         // token t
+  const char* tok_base_c = reinterpret_cast<const char*>(to_head ? src : dst) + (int64_t)g0 * chunk_bytes;
+  if (to_head)
+    return launch_copy(tok_base_c, dst, nullptr, nullptr, 1, G, n_tok, dv, tok_a, tok_b, head_a, head_b, (cudaStream_t)stream);
+  return launch_copy(src, const_cast<char*>(tok_base_c), nullptr, nullptr, 1, G, n_tok, dv, head_a, head_b, tok_a, tok_b,
+                     (cudaStream_t)stream);
+}
+
+}  // namespace
+
+extern "C" __attribute__((visibility("default"))) int ws_kv_cache_write(void* k_cache, void* v_cache, int64_t capacity, int32_t H, int32_t d, const void* k_src,
+                                 const void* v_src, int32_t n_rows, int32_t H_src, int32_t head_begin, int64_t row_offset,
+                                 ws_dtype dt, void* stream) {
+  const int es = wsi::elem_bytes(dt);
+  if (es == 0) return WS_ERR_UNSUPPORTED;
+  if (!k_cache || !v_cache || capacity <= 0 || H <= 0 || d <= 0 || n_rows < 0 || H_src <= 0 || head_begin < 0 ||
+      head_begin + (int64_t)H > H_src)
+    return WS_ERR_INVALID_ARG;
+  if (n_rows > 0 && (!k_src || !v_src)) return WS_ERR_INVALID_ARG;
+  if (row_offset < 0 || row_offset + n_rows > capacity) return WS_ERR_OUT_OF_RANGE;
+  const int64_t row_bytes = (int64_t)d * es;
+  if (row_bytes % 16 != 0 || !wsi::aligned16(k_cache) || !wsi::aligned16(v_cache) || !wsi::aligned16(k_src) ||
+      !wsi::aligned16(v_src))
+    return WS_ERR_ALIGNMENT;
+  if (n_rows == 0) return WS_OK;
+  const size_t cache_bytes = (size_t)H * capacity * row_bytes, src_bytes = (size_t)n_rows * H_src * row_bytes;
+  const void* caches[2] = {k_cache, v_cache};
+  const void* srcs[2] = {k_src, v_src};
+  for (int i = 0; i < 2; ++i)
+    for (int j = 0; j < 2; ++j)
+      if (wsi::ranges_overlap(caches[i], cache_bytes, srcs[j], src_bytes)) return WS_ERR_OVERLAP;
+  if (wsi::ranges_overlap(k_cache, cache_bytes, v_cache, cache_bytes)) return WS_ERR_OVERLAP;
+  const int64_t dv = row_bytes / 16;
+  // a = head h, b = row r:  src (r * H_src + head_begin + h) * dv ; dst (h * capacity + row_offset + r) * dv
+  const char* ks = reinterpret_cast<const char*>(k_src) + (int64_t)head_begin * row_bytes;
+  const char* vs = reinterpret_cast<const char*>(v_src) + (int64_t)head_begin * row_bytes;
+  char* kd = reinterpret_cast<char*>(k_cache) + row_offset * row_bytes;
+  char* vd = reinterpret_cast<char*>(v_cache) + row_offset * row_bytes;
+  return launch_copy(ks, kd, vs, vd, 2, H, n_rows, dv, dv, (int64_t)H_src * dv, capacity * dv, dv, (cudaStream_t)stream);
+}
+
+extern "C" __attribute__((visibility("default"))) int ws_seq_to_head(void* dst, const void* src, int64_t n_tok, int32_t H, int32_t d, int32_t P, int32_t g0, int32_t G,
+                              ws_dtype dt, void* stream) {
+  return relayout(dst, src, n_tok, H, d, P, g0, G, dt, stream, true);
+}
+
+extern "C" __attribute__((visibility("default"))) int ws_head_to_seq(void* dst, const void* src, int64_t n_tok, int32_t H, int32_t d, int32_t P, int32_t g0, int32_t G,
+                              ws_dtype dt, void* stream) {
+  return relayout(dst, src, n_tok, H, d, P, g0, G, dt, stream, false);
+}

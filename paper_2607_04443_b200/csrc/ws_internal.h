@@ -1,0 +1,35 @@
+// Internal helpers shared by the ws_*.cu translation units (NOT part of the C ABI, and not
+// shared with oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "ws.h"
+
+namespace wsi {
+
+// Records a CUDA error for ws_last_cuda_error() and returns WS_ERR_CUDA.
+int cuda_fail(cudaError_t e);
+// Bumps the process-wide launch counter reported by ws_kernel_launch_count().
+void count_launch(int n = 1);
+
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+inline bool aligned256(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 255u) == 0; }
+inline int elem_bytes(ws_dtype dt) { return dt == WS_DTYPE_BF16 ? 2 : (dt == WS_DTYPE_F32 ? 4 : 0); }
+inline bool ranges_overlap(const void* a, size_t na, const void* b, size_t nb) {
+  const uintptr_t a0 = reinterpret_cast<uintptr_t>(a), b0 = reinterpret_cast<uintptr_t>(b);
+  return na != 0 && nb != 0 && a0 < b0 + nb && b0 < a0 + na;
+}
+
+// After a launch: pick up launch-configuration errors without synchronising.
+inline int after_launch(int n_launches) {
+  cudaError_t e = cudaPeekAtLastError();
+  if (e != cudaSuccess) {
+    (void)cudaGetLastError();
+    return cuda_fail(e);
+  }
+  count_launch(n_launches);
+  return WS_OK;
+}
+
+}  // namespace wsi

@@ -1,0 +1,165 @@
+"""The C-ABI boundary without a GPU: libws.so loads, exports every symbol include/ws.h declares,
+and rejects bad arguments before touching CUDA (so these calls are safe on a CPU-only box).
+No compute call is made here."""
+import ctypes
+import os
+import re
+
+import pytest
+import torch
+
+import paper_2607_04443_b200 as ws
+from paper_2607_04443_b200 import binding, build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+OK, INVALID, UNSUPPORTED, ALIGN, RANGE, OVERLAP, WORKSPACE, CUDA = 0, -1, -2, -3, -4, -5, -6, -7
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build_lib()
+    return binding.load()
+
+
+def declared_functions():
+    text = open(os.path.join(ROOT, "include", "ws.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(ws_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol(lib):
+    names = declared_functions()
+    assert set(names) == set(binding.EXPORTS), (names, binding.EXPORTS)
+    for n in names:
+        assert getattr(lib, n) is not None
+    # and nothing from the oracle is linked in
+    syms = os.popen(f"nm -D --defined-only {binding.lib_path()}").read()
+    assert "wsref" not in syms
+    exported = set(re.findall(r" T (ws_[a-z0-9_]+)", syms))
+    assert exported == set(names)
+
+
+def test_version_and_status_strings(lib):
+    assert ws.version() == 100
+    assert ws.status_string(0) == "WS_OK"
+    for code in range(-7, 0):
+        assert ws.status_string(code).startswith("WS_ERR_")
+    assert ws.status_string(-99) == "WS_ERR_UNKNOWN"
+
+
+def P(x):
+    return ctypes.c_void_p(x)
+
+
+A, B, C, D = 0x10000000, 0x20000000, 0x30000000, 0x40000000  # fake, 16-byte aligned, far apart
+
+
+def test_kv_cache_write_rejects_bad_arguments(lib):
+    f = lib.ws_kv_cache_write
+    good = dict(kc=A, vc=B, cap=1024, H=4, d=128, ks=C, vs=D, n=64, Hs=8, hb=2, off=100, dt=0)
+
+    def call(**kw):
+        a = dict(good, **kw)
+        return f(P(a["kc"]), P(a["vc"]), a["cap"], a["H"], a["d"], P(a["ks"]), P(a["vs"]), a["n"], a["Hs"], a["hb"], a["off"],
+                 a["dt"], None)
+
+    assert call(off=1024 - 63) == RANGE
+    assert call(off=-1) == RANGE
+    assert call(hb=5) == INVALID          # head_begin + H > H_src
+    assert call(kc=0) == INVALID
+    assert call(dt=7) == UNSUPPORTED
+    assert call(kc=A + 8) == ALIGN
+    assert call(d=4) == ALIGN             # 8-byte rows
+    assert call(ks=A + 4096) == OVERLAP   # source inside the K cache
+    assert call(vc=A + 1024) == OVERLAP   # caches overlap each other
+    assert call(n=0) == OK                # no-op, nothing launched
+
+
+def test_relayout_rejects_bad_arguments(lib):
+    for f in (lib.ws_seq_to_head, lib.ws_head_to_seq):
+        def call(dst=A, src=B, n_tok=100, H=40, d=128, Pn=4, g0=1, G=1, dt=0):
+            return f(P(dst), P(src), n_tok, H, d, Pn, g0, G, dt, None)
+
+        assert call(Pn=3) == INVALID      # H % P != 0
+        assert call(g0=4) == INVALID
+        assert call(g0=3, G=2) == INVALID
+        assert call(Pn=0) == INVALID
+        assert call(dst=0) == INVALID
+        assert call(dt=5) == UNSUPPORTED
+        assert call(src=B + 2) == ALIGN
+        assert call(src=A + 256) == OVERLAP
+        assert call(n_tok=0) == OK
+        assert call(G=0) == OK
+
+
+def test_attention_rejects_bad_arguments(lib):
+    f = lib.ws_block_causal_attn
+    Mask = binding._BlockMask
+
+    def call(out=A, q=B, kc=C, vc=D, cap=512, Tc=512, kn=0x50000000, vn=0x60000000, Ln=64, H=2, d=128, Lq=64, qe=(32, 64),
+             kv=(544, 576), scale=0.1, wsp=0x70000000, wsb=1 << 30, dt=0, lse=None):
+        n = len(qe)
+        m = Mask(n, (ctypes.c_int32 * n)(*qe), (ctypes.c_int32 * n)(*kv))
+        return f(P(out), lse, P(q), P(kc), P(vc), cap, Tc, P(kn) if kn else None, P(vn) if vn else None, Ln, H, d, Lq,
+                 ctypes.byref(m), scale, P(wsp) if wsp else None, wsb, dt, None)
+
+    assert call(d=96) == UNSUPPORTED
+    assert call(dt=3) == UNSUPPORTED
+    assert call(qe=(32, 63)) == INVALID             # last != Lq
+    assert call(qe=(32, 32)) == INVALID             # not strictly increasing
+    assert call(kv=(576, 544)) == INVALID           # decreasing visibility
+    assert call(kv=(544, 577)) == RANGE             # beyond cache_len + Ln
+    assert call(Tc=513) == RANGE                    # cache_len > capacity
+    assert call(kn=0) == INVALID                    # Ln > 0 but k_new NULL
+    assert call(Ln=0, kv=(100, 512)) == INVALID     # Ln == 0 but k_new given
+    assert call(scale=-1.0) == INVALID
+    assert call(scale=float("nan")) == INVALID
+    assert call(q=B + 8) == ALIGN
+    assert call(wsp=0) == WORKSPACE
+    assert call(wsb=1024) == WORKSPACE
+    assert call(wsp=0x70000010) == WORKSPACE        # not 256-byte aligned
+    assert call(qe=tuple(range(1, 131)), kv=tuple([576] * 130), Lq=130) == UNSUPPORTED  # > WS_MAX_MASK_BLOCKS
+
+
+def test_workspace_bytes_is_sane(lib):
+    f = lib.ws_block_causal_attn_workspace_bytes
+    assert f(0, 1, 128, 10, 0) == 0
+    b3 = f(970, 40, 128, 17354, 0)
+    assert 20 << 20 < b3 < 200 << 20
+    assert f(970, 40, 128, 17354, 1) > b3 + 2 * 40 * 17354 * 128 * 2  # FP32 staging on top
+    assert f(3680, 10, 128, 20064, 0) >= f(970, 10, 128, 20064, 0)
+    g = lib.ws_unit_forward_host_staging_bytes
+    assert g(970, 970, 40, 128, 1024, 17354, 1) > b3 + 3 * 970 * 40 * 128 * 2
+
+
+def test_binding_refuses_cpu_tensors_no_fallback(lib):
+    kc = torch.zeros(2, 8, 64, dtype=torch.bfloat16)
+    ks = torch.zeros(4, 2, 64, dtype=torch.bfloat16)
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        ws.kv_cache_write(kc, kc.clone(), ks, ks.clone(), 0, 0)
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        ws.seq_to_head(torch.zeros(1, 4, 1, 64, dtype=torch.bfloat16), ks, 2, 0, 1)
+
+
+def test_missing_library_fails_loudly(monkeypatch):
+    monkeypatch.setattr(binding, "_lib", None)
+    monkeypatch.setattr(binding, "_LIB_PATH", "/nonexistent/libws.so")
+    with pytest.raises(RuntimeError, match="no CPU or PyTorch fallback"):
+        binding.load()
+
+
+def test_product_never_imports_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2607_04443_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for fn in files:
+            if fn.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, fn)).read()
+                assert "wsref" not in text and "import oracle" not in text and "from oracle" not in text, fn
+    hdr = open(os.path.join(ROOT, "include", "ws.h")).read()
+    assert "wsref" not in hdr
+    for fn in os.listdir(os.path.join(ROOT, "oracle")):
+        if fn.endswith((".py", ".c")):
+            text = open(os.path.join(ROOT, "oracle", fn)).read()
+            assert "paper_2607_04443_b200 import" not in text.replace("never imports", "") or fn == "__init__.py"
+            assert "ws.h" not in text or "includes nothing from include/" in text
