@@ -1,0 +1,515 @@
+#!/usr/bin/env python
+"""bench.py -- the 640x368 unit (BASELINE.json configs[2], "cfg3") through the whole hot path.
+
+One STEP = one pass of every row of SURVEY.md section 8(a) over one unit of synthetic input:
+    a1 ws_kv_cache_write (1024-row K/V slice into the 16384-row cache)
+    a2 ws_seq_to_head on Q, K_new, V_new          (P = 1: one GPU holds all 40 heads)
+    a3 ws_block_causal_attn (970 queries x 40 heads x 17354 keys, d = 128, BF16)
+    a4 ws_head_to_seq on O
+metric = block-causal unit attention TFLOP/s = algorithmic attention flops (visible pairs only)
+per step / step time.  `value` has inputs resident in HBM; `e2e` goes through the C-ABI host entry
+ws_unit_forward_host with pinned HOST buffers (H2D + kernels + D2H inside the timed region).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-aux]
+
+N > 1 (torchrun): replicas only -- every rank runs the same unit on its own GPU, no data-path
+collective (north_star: single-GPU share); value = sum of units / max time.
+--impl reference times the CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2607_04443_b200 import workloads as wl  # noqa: E402
+
+WORKLOAD = "cfg3"
+METRIC = "block_causal_unit_attention_tflops"
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        p["_source"] = "measured"
+        return p
+    p = dict(FALLBACK_PEAKS)
+    p["_source"] = "fallback"
+    return p
+
+
+# ------------------------------------------------------------------------------------------------
+# multi-rank plumbing (replicas only): barrier + max-over-ranks time + summed units
+# ------------------------------------------------------------------------------------------------
+def dist_setup(n_gpus: int, backend: str = "nccl"):
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world == 1:
+        return 0, 1, None
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    dist.init_process_group(backend=backend)
+    return dist.get_rank(), dist.get_world_size(), dist
+
+
+def aggregate_over_ranks(local_ms: float, local_units: float, dist, device):
+    """(max time over ranks, total units over ranks).  Works with nccl (GPU tensors) and gloo (CPU)."""
+    if dist is None:
+        return local_ms, local_units
+    import torch
+    t = torch.tensor([local_ms], dtype=torch.float64, device=device)
+    u = torch.tensor([local_units], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks during the timed region
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.path = None
+
+    def __enter__(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.QUERY}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+        return self
+
+    def __exit__(self, *exc):
+        if self.proc is not None:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if not self.path or not os.path.exists(self.path):
+            return out
+        sm, reasons, mx, pw = [], set(), None, []
+        for line in open(self.path):
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx = float(f[1])
+                pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        os.unlink(self.path)
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=mx, reasons=sorted(reasons), samples=len(sm),
+                       power_w_max=max(pw))
+        return out
+
+
+# ------------------------------------------------------------------------------------------------
+# our arm
+# ------------------------------------------------------------------------------------------------
+def dev_bf16(a):
+    import torch
+    return torch.from_numpy(wl.bf16_bits(a).view(np.int16)).cuda().view(torch.bfloat16)
+
+
+def pinned_bf16(a):
+    import torch
+    return torch.from_numpy(wl.bf16_bits(a).view(np.int16)).view(torch.bfloat16).pin_memory()
+
+
+class UnitOnDevice:
+    """cfg3 inputs resident in HBM + the per-step call sequence (a1..a4)."""
+
+    def __init__(self, cfg, n_sets: int = 2):
+        import torch
+        import paper_2607_04443_b200 as ws
+        self.ws, self.cfg, self.torch = ws, cfg, torch
+        x = wl.generate(cfg)
+        self.x = x
+        self.kc, self.vc = dev_bf16(x["k_cache"]), dev_bf16(x["v_cache"])
+        L, H, d = cfg.Lq, cfg.H, cfg.d
+        self.sets = []
+        for s in range(n_sets):  # distinct per-unit inputs, rotated so they do not sit in L2 by construction
+            roll = s * 7
+            mk = lambda a: dev_bf16(np.roll(a, roll, axis=0))
+            self.sets.append(dict(ks=mk(x["k_slice"]), vs=mk(x["v_slice"]), q=mk(x["q"][0]), kn=mk(x["k_new"][0]),
+                                  vn=mk(x["v_new"][0])))
+        e = lambda: torch.empty((1, L, H, d), dtype=torch.bfloat16, device="cuda")
+        self.q_h, self.kn_h, self.vn_h, self.o_h = e(), e(), e(), e()
+        self.out = torch.empty((L, H, d), dtype=torch.bfloat16, device="cuda")
+        self.wsp = torch.empty(ws.block_causal_attn_workspace_bytes(L, H, d, cfg.cache_len + cfg.Ln), dtype=torch.uint8,
+                               device="cuda")
+        self.phase_events = []
+
+    def step(self, i: int, record: bool = False):
+        ws, cfg, torch = self.ws, self.cfg, self.torch
+        s = self.sets[i % len(self.sets)]
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(5)] if record else None
+        if record: ev[0].record()
+        ws.kv_cache_write(self.kc, self.vc, s["ks"], s["vs"], 0, cfg.write_offset)
+        if record: ev[1].record()
+        ws.seq_to_head(self.q_h, s["q"], 1, 0, 1)
+        ws.seq_to_head(self.kn_h, s["kn"], 1, 0, 1)
+        ws.seq_to_head(self.vn_h, s["vn"], 1, 0, 1)
+        if record: ev[2].record()
+        ws.block_causal_attn(self.o_h[0], self.q_h[0], self.kc, self.vc, cfg.cache_len, self.kn_h[0], self.vn_h[0],
+                             cfg.q_block_end, cfg.kv_visible, cfg.softmax_scale, self.wsp)
+        if record: ev[3].record()
+        ws.head_to_seq(self.out, self.o_h, 1, 0, 1)
+        if record:
+            ev[4].record()
+            self.phase_events.append(ev)
+
+    def phase_ms(self):
+        names = ("cache_write", "seq_to_head_x3", "attention", "head_to_seq")
+        acc = {n: [] for n in names}
+        for ev in self.phase_events:
+            for k, n in enumerate(names):
+                acc[n].append(ev[k].elapsed_time(ev[k + 1]))
+        return {n: statistics.mean(v) for n, v in acc.items() if v}
+
+
+def timed_region(fn, steps, warmup, dist):
+    import torch
+    import paper_2607_04443_b200 as ws
+    for i in range(warmup):
+        fn(i, False)
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    n0 = ws.kernel_launch_count()
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record()
+    for i in range(steps):
+        fn(warmup + i, True)
+    t1.record()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    return t0.elapsed_time(t1), ws.kernel_launch_count() - n0
+
+
+def e2e_host(cfg, x, steps, warmup, dist):
+    """Same unit through ws_unit_forward_host: pinned host inputs -> device -> kernels -> pinned host output."""
+    import torch
+    import paper_2607_04443_b200 as ws
+    kc, vc = dev_bf16(x["k_cache"]), dev_bf16(x["v_cache"])
+    qh = pinned_bf16(x["q"][0][None])
+    knh, vnh = pinned_bf16(x["k_new"][0][None]), pinned_bf16(x["v_new"][0][None])
+    ksh, vsh = pinned_bf16(x["k_slice"]), pinned_bf16(x["v_slice"])
+    outh = torch.zeros_like(qh).pin_memory()
+    staging = torch.empty(ws.unit_forward_host_staging_bytes(cfg.Lq, cfg.Ln, cfg.H, cfg.d, cfg.write_rows,
+                                                             cfg.cache_len + cfg.Ln, 1), dtype=torch.uint8, device="cuda")
+    h2d = sum(t.numel() * 2 for t in (qh, knh, vnh, ksh, vsh))
+    d2h = outh.numel() * 2
+
+    def fn(i, _rec):
+        ws.unit_forward_host(outh, qh, knh, vnh, kc, vc, ksh, vsh, cfg.write_offset, cfg.cache_len, cfg.softmax_scale, staging)
+        torch.cuda.current_stream().synchronize()  # the user reads the result on the host every step
+
+    ms, _ = timed_region(fn, steps, warmup, dist)
+    assert torch.isfinite(outh.float()).all()
+    return ms, h2d, d2h
+
+
+def bandwidth_aux(peaks):
+    """Cache-write and relayout GB/s with an L2-defeating rotation (footprint > 4 x L2), SURVEY.md 8(d)."""
+    import torch
+    import paper_2607_04443_b200 as ws
+    res = {}
+    g = torch.Generator(device="cuda").manual_seed(5)
+    rnd = lambda *s: torch.randn(*s, generator=g, device="cuda", dtype=torch.float32).to(torch.bfloat16)
+
+    def time_calls(calls, reps=3):
+        best = None
+        for _ in range(reps):
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for c in calls:
+                c()
+            b.record()
+            torch.cuda.synchronize()
+            ms = a.elapsed_time(b) / len(calls)
+            best = ms if best is None else min(best, ms)
+        return best
+
+    # a1 at cfg3 size: 1024 rows x 40 heads; 64 destination windows in a 65536-row cache, 24 source sets
+    H, d, n, cap = 40, 128, 1024, 65536
+    kc, vc = torch.empty((H, cap, d), dtype=torch.bfloat16, device="cuda"), torch.empty((H, cap, d), dtype=torch.bfloat16, device="cuda")
+    srcs = [(rnd(n, H, d), rnd(n, H, d)) for _ in range(24)]
+    calls = [(lambda i=i: ws.kv_cache_write(kc, vc, srcs[i % 24][0], srcs[i % 24][1], 0, (i % 64) * n)) for i in range(192)]
+    time_calls(calls[:8], 1)
+    ms = time_calls(calls)
+    byts = 2 * 2 * n * H * d * 2
+    res["cache_write_cfg3"] = {"us": ms * 1e3, "gbs": byts / ms / 1e6, "bytes": byts, "frac_hbm": byts / ms / 1e6 / peaks["hbm_gbs"]}
+    # a1 saturating variant: one call writing all 65536 rows (1.34 GB payload per tensor pair)
+    big_k, big_v = rnd(8192, H, d), rnd(8192, H, d)
+    calls = [(lambda i=i: ws.kv_cache_write(kc, vc, big_k, big_v, 0, (i % 8) * 8192)) for i in range(16)]
+    ms = time_calls(calls)
+    byts = 2 * 2 * 8192 * H * d * 2
+    res["cache_write_8192rows"] = {"us": ms * 1e3, "gbs": byts / ms / 1e6, "bytes": byts, "frac_hbm": byts / ms / 1e6 / peaks["hbm_gbs"]}
+    del kc, vc, srcs, big_k, big_v
+    # a2/a4 at cfg4 size: [3680, 40, 128], P = 4, G = 1; 56 distinct source/destination pairs (> 4 x L2)
+    L, P = 3680, 4
+    srcs = [rnd(L, H, d) for _ in range(28)]
+    dsts = [torch.empty((1, L, H // P, d), dtype=torch.bfloat16, device="cuda") for _ in range(56)]
+    calls = [(lambda i=i: ws.seq_to_head(dsts[i % 56], srcs[i % 28], P, i % 4, 1)) for i in range(224)]
+    time_calls(calls[:8], 1)
+    ms = time_calls(calls)
+    byts = 2 * L * (H // P) * d * 2
+    res["seq_to_head_cfg4"] = {"us": ms * 1e3, "gbs": byts / ms / 1e6, "bytes": byts, "frac_hbm": byts / ms / 1e6 / peaks["hbm_gbs"]}
+    calls = [(lambda i=i: ws.head_to_seq(srcs[i % 28], dsts[i % 56], P, i % 4, 1)) for i in range(224)]
+    ms = time_calls(calls)
+    res["head_to_seq_cfg4"] = {"us": ms * 1e3, "gbs": byts / ms / 1e6, "bytes": byts, "frac_hbm": byts / ms / 1e6 / peaks["hbm_gbs"]}
+    # saturating variant: G = P full pack of a 32x longer sequence (1.2 GB read + 1.2 GB written)
+    Lb = 3680 * 32
+    src = rnd(Lb, H, d)
+    dst = torch.empty((P, Lb, H // P, d), dtype=torch.bfloat16, device="cuda")
+    calls = [lambda: ws.seq_to_head(dst, src, P, 0, P)] * 4
+    ms = time_calls(calls)
+    byts = 2 * Lb * H * d * 2
+    res["seq_to_head_G4_1.2GB"] = {"us": ms * 1e3, "gbs": byts / ms / 1e6, "bytes": byts, "frac_hbm": byts / ms / 1e6 / peaks["hbm_gbs"]}
+    calls = [lambda: ws.head_to_seq(src, dst, P, 0, P)] * 4
+    ms = time_calls(calls)
+    res["head_to_seq_G4_1.2GB"] = {"us": ms * 1e3, "gbs": byts / ms / 1e6, "bytes": byts, "frac_hbm": byts / ms / 1e6 / peaks["hbm_gbs"]}
+    return res
+
+
+def attention_aux(peaks):
+    """Attention alone on the other BASELINE.json shapes (device-generated N(0,1) inputs), and the
+    config-5 unit (cache write + 8 steps) under one CUDA graph: ms per unit."""
+    import torch
+    import paper_2607_04443_b200 as ws
+    res = {}
+    g = torch.Generator(device="cuda").manual_seed(6)
+    rnd = lambda std, *s: (torch.randn(*s, generator=g, device="cuda", dtype=torch.float32) * std).to(torch.bfloat16)
+    for name in ("cfg2", "cfg4", "cfg5"):
+        cfg = wl.CONFIGS[name]
+        L, H, d = cfg.Lq, cfg.H, cfg.d
+        kc, vc = rnd(cfg.kv_std, H, cfg.capacity, d), rnd(cfg.kv_std, H, cfg.capacity, d)
+        q, kn, vn = rnd(cfg.q_premul, L, H, d), rnd(cfg.kv_std, L, H, d), rnd(cfg.kv_std, L, H, d)
+        out = torch.empty_like(q)
+        wsp = torch.empty(ws.block_causal_attn_workspace_bytes(L, H, d, cfg.cache_len + cfg.Ln), dtype=torch.uint8, device="cuda")
+        call = lambda: ws.block_causal_attn(out, q, kc, vc, cfg.cache_len, kn, vn, cfg.q_block_end, cfg.kv_visible,
+                                            cfg.softmax_scale, wsp)
+        for _ in range(3):
+            call()
+        torch.cuda.synchronize()
+        reps = 10
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(reps):
+            call()
+        b.record()
+        torch.cuda.synchronize()
+        ms = a.elapsed_time(b) / reps
+        tf = cfg.attn_flops() / ms / 1e9
+        res[name] = {"attention_ms": ms, "tflops": tf, "frac_bf16_peak": tf / peaks["bf16_tflops"]}
+        if name == "cfg5":
+            ks, vs = rnd(cfg.kv_std, cfg.write_rows, H, d), rnd(cfg.kv_std, cfg.write_rows, H, d)
+            qs = [rnd(1.0, L, H, d) for _ in range(cfg.steps)]
+            outs = [torch.empty_like(q) for _ in range(cfg.steps)]
+            stream = torch.cuda.Stream()
+            graph = torch.cuda.CUDAGraph()
+            torch.cuda.synchronize()
+            with torch.cuda.graph(graph, stream=stream):
+                ws.kv_cache_write(kc, vc, ks, vs, 0, cfg.write_offset)
+                for s in range(cfg.steps):
+                    ws.block_causal_attn(outs[s], qs[s], kc, vc, cfg.cache_len, kn, vn, cfg.q_block_end, cfg.kv_visible,
+                                         cfg.softmax_scale, wsp)
+            graph.replay()
+            torch.cuda.synchronize()
+            a.record()
+            for _ in range(3):
+                graph.replay()
+            b.record()
+            torch.cuda.synchronize()
+            ms_unit = a.elapsed_time(b) / 3
+            tf = cfg.attn_flops() * cfg.steps / ms_unit / 1e9
+            res["cfg5_unit_graph"] = {"ms_per_unit": ms_unit, "steps": cfg.steps, "tflops": tf,
+                                      "frac_bf16_peak_sustained": tf / peaks["bf16_tflops_sustained"],
+                                      "paper_budget_ms_per_unit_all_layers": 160.0}
+        del kc, vc
+    return res
+
+
+def cpu_oracle_sample(cfg, x, target_seconds: float = 12.0):
+    """The oracle as it stands on a bounded sample of (row, head) pairs of this workload."""
+    from oracle import wsref
+    kc, vc = x["k_cache"].copy(), x["v_cache"].copy()
+    wsref.kv_cache_write(kc, vc, x["k_slice"], x["v_slice"], 0, cfg.write_offset)
+    args = (x["q"][0], kc, vc, cfg.cache_len, x["k_new"][0], x["v_new"][0], cfg.q_block_end, cfg.kv_visible, cfg.softmax_scale)
+    flops_per_row = 4 * cfg.kv_visible[0] * cfg.d
+    rows, heads = wl.sample_pairs(cfg, 256, seed=99)
+    t = time.perf_counter()
+    wsref.block_causal_attn_rows(*args, rows, heads)
+    dt = time.perf_counter() - t
+    n = int(max(256, min(cfg.Lq * cfg.H, target_seconds / (dt / len(rows)))))
+    rows, heads = wl.sample_pairs(cfg, n, seed=100)
+    t = time.perf_counter()
+    wsref.block_causal_attn_rows(*args, rows, heads)
+    dt = time.perf_counter() - t
+    return {"value": flops_per_row * len(rows) / dt / 1e12, "unit": "TFLOP/s", "cores": wsref.num_threads(), "kind": "oracle",
+            "sample": f"{len(rows)} of {cfg.Lq * cfg.H} (row, head) outputs of {cfg.name}, FP64, {dt:.1f} s",
+            "seconds": dt}, args
+
+
+def run_ours(args):
+    import torch
+    import paper_2607_04443_b200 as ws
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product has no CPU fallback (use --impl reference for the oracle)")
+    rank, world, dist = dist_setup(args.gpus)
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    ws.load()
+    peaks = load_peaks()
+    cfg = wl.CONFIGS[WORKLOAD]
+    unit = UnitOnDevice(cfg)
+    flops = cfg.attn_flops()
+
+    with ClockSampler(local) as clk:
+        ms_local, launches_timed = timed_region(unit.step, args.steps, args.warmup, dist)
+    clocks = clk.summary()
+    ms, units = aggregate_over_ranks(ms_local, float(args.steps), dist, "cuda")
+    value = flops * units / ms / 1e9  # TFLOP/s, whole job
+    phases = unit.phase_ms()
+    attn_ms = phases["attention"]
+    achieved = flops / attn_ms / 1e9
+
+    e2e_steps = max(3, args.steps // 4)
+    if args.kernels_only:
+        e2e_ms_local, h2d, d2h = float("nan"), 0, 0
+    else:
+        e2e_ms_local, h2d, d2h = e2e_host(cfg, unit.x, e2e_steps, args.warmup, dist)
+    e2e_ms, e2e_units = aggregate_over_ranks(e2e_ms_local, float(e2e_steps), dist, "cuda")
+
+    line = {
+        "metric": METRIC, "value": value, "unit": "TFLOP/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+        "data": "synthetic", "impl": "ours",
+        "config": {"workload": "cfg3: 640x368 unit, 970 queries (920 video + 50 audio) x 40 heads x d128, cache 16384 + own 970 keys, "
+                               "1024-row K/V slice written first; step = cache write + 3x seq->head + attention + head->seq (P=1)",
+                   "l2_policy": "inputs larger than L2 (335 MB K/V cache per step vs 126 MB L2) and two rotating input sets",
+                   "seed": cfg.seed, "flops_per_step": flops, "replicas": world},
+        "e2e": {"value": flops * e2e_units / e2e_ms / 1e9, "unit": "TFLOP/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": e2e_ms / e2e_steps, "api": "ws_unit_forward_host (pinned host buffers)"},
+        "gpu_launches": launches_timed,
+        "clocks": clocks,
+        "roofline": {"bound": "tensor", "kernel": "attn_fwd_kernel<128> (+ combine, timed together)", "achieved": achieved,
+                     "peak": peaks["bf16_tflops"], "unit": "TFLOP/s", "frac": achieved / peaks["bf16_tflops"],
+                     "peak_source": f"{peaks['_source']} burst (cuBLAS bf16)", "frac_of_sustained": achieved / peaks["bf16_tflops_sustained"],
+                     "frac_of_nominal_2250": achieved / 2250.0, "traffic": read_traffic(), "launch_ms": attn_ms},
+        "phases_ms": phases,
+    }
+    if rank == 0 and world == 1 and not args.kernels_only:
+        cpu, _ = cpu_oracle_sample(cfg, unit.x)
+        line["cpu_baseline"] = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        if not args.no_aux:
+            del unit
+            torch.cuda.empty_cache()
+            line["aux"] = {"bandwidth": bandwidth_aux(peaks), "attention": attention_aux(peaks),
+                           "hbm_peak_gbs": peaks["hbm_gbs"], "peak_source": peaks["_source"]}
+    if rank == 0:
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def read_traffic():
+    """DRAM bytes per attention launch from the committed ncu capture (profiles/), or None."""
+    path = os.path.join(ROOT, "profiles", "attn_traffic.json")
+    if os.path.exists(path):
+        try:
+            return json.load(open(path)).get("dram_bytes_per_launch")
+        except Exception:
+            return None
+    return None
+
+
+# ------------------------------------------------------------------------------------------------
+# reference arm: the CPU oracle, as it stands, on a bounded sample per step
+# ------------------------------------------------------------------------------------------------
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return  # under torchrun only rank 0 runs the oracle; the others exit 0 without work
+    from oracle import wsref
+    cfg = wl.CONFIGS[WORKLOAD]
+    x = wl.generate(cfg)
+    kc, vc = x["k_cache"].copy(), x["v_cache"].copy()
+    wsref.kv_cache_write(kc, vc, x["k_slice"], x["v_slice"], 0, cfg.write_offset)
+    a = (x["q"][0], kc, vc, cfg.cache_len, x["k_new"][0], x["v_new"][0], cfg.q_block_end, cfg.kv_visible, cfg.softmax_scale)
+    n_rows = 192  # per step: a bounded sample (rows are independent); whole run stays within minutes
+    flops_per_row = 4 * cfg.kv_visible[0] * cfg.d
+    for i in range(args.warmup):
+        rows, heads = wl.sample_pairs(cfg, n_rows, seed=i)
+        wsref.block_causal_attn_rows(*a, rows, heads)
+    n_done, t0 = 0, time.perf_counter()
+    for i in range(args.steps):
+        rows, heads = wl.sample_pairs(cfg, n_rows, seed=1000 + i)
+        wsref.block_causal_attn_rows(*a, rows, heads)
+        n_done += len(rows)
+    dt = time.perf_counter() - t0
+    value = flops_per_row * n_done / dt / 1e12
+    sample = f"{n_done // max(args.steps, 1)} (row, head) outputs of cfg3 per step, FP64 oracle"
+    line = {"metric": METRIC, "value": value, "unit": "TFLOP/s", "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt * 1e3 / max(args.steps, 1), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "impl": "reference",
+            "config": {"workload": "cfg3: 640x368 unit (bounded sample of its (row, head) outputs per step)", "seed": cfg.seed},
+            "cpu_baseline": {"value": value, "unit": "TFLOP/s", "cores": wsref.num_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": "TFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=40)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--no-aux", action="store_true", help="skip the per-kernel bandwidth / other-config measurements")
+    ap.add_argument("--kernels-only", action="store_true",
+                    help="profiling mode: only the device-resident timed steps (no e2e, cpu_baseline or aux legs)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
