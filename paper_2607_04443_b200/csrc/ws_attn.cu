@@ -22,9 +22,19 @@
 
 #include <cstring>
 #include <mutex>
+#include <type_traits>
 
 #include "ws_internal.h"
 #include "ws_ptx.cuh"
+
+#ifdef WS_ATTN_TRACE
+__device__ unsigned long long* g_trace_ptr = nullptr;
+#define WS_TRACE_DECL(role, cond) unsigned long long* trc_ = (blockIdx.x == 5 && g_trace_ptr && (cond)) ? g_trace_ptr + (role) * 8192 : nullptr; int trc_i_ = 0;
+#define WS_TRACE(ev) do { if (trc_ && trc_i_ < 8190) trc_[trc_i_++] = ((unsigned long long)(ev) << 48) | ((unsigned long long)clock64() & 0xffffffffffffull); } while (0)
+#else
+#define WS_TRACE_DECL(role, cond)
+#define WS_TRACE(ev)
+#endif
 
 namespace {
 
@@ -39,6 +49,10 @@ constexpr int kTmemCols = 512;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kRescaleThreshold = 8.0f;  // log2 units: P stays below 2^8
+#ifndef WS_POLY_OF4
+#define WS_POLY_OF4 1
+#endif
+constexpr int kPolyOf4 = WS_POLY_OF4;  // of every 4 pairs of exponentials, this many run on the FMA pipe instead of MUFU
 
 struct alignas(64) Params {
   CUtensorMap map_q, map_kn, map_vn, map_kc, map_vc;
@@ -140,7 +154,7 @@ struct Cfg {
 struct Barriers {
   uint64_t kv_full[kStages], kv_empty[kStages];
   uint64_t q_full, q_empty;
-  uint64_t s_full[2], p_full[2], o_done[2];
+  uint64_t s_full[2], p_lo[2], p_hi[2], o_done[2];  // p_lo / p_hi: P of keys [0,64) / [64,128) is in TMEM
   uint32_t tmem_base;
 };
 
@@ -157,7 +171,9 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
   Sched& sched = *reinterpret_cast<Sched*>(smem + C::kSmemQ + C::kSmemKV + 256);
   static_assert(sizeof(Barriers) <= 256, "barrier block");
 
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  // the warp index goes through a shuffle so that ptxas knows it is warp-uniform: the TMA and MMA
+  // warps then run in uniform control flow and their descriptors live in uniform registers
+  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < kStages; ++i) {
@@ -168,7 +184,8 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
     ptx::mbar_init(ptx::smem_u32(&bar.q_empty), 1);
     for (int t = 0; t < 2; ++t) {
       ptx::mbar_init(ptx::smem_u32(&bar.s_full[t]), 1);
-      ptx::mbar_init(ptx::smem_u32(&bar.p_full[t]), kBlockM);
+      ptx::mbar_init(ptx::smem_u32(&bar.p_lo[t]), kBlockM);
+      ptx::mbar_init(ptx::smem_u32(&bar.p_hi[t]), kBlockM);
       ptx::mbar_init(ptx::smem_u32(&bar.o_done[t]), 1);
     }
     ptx::fence_mbar_init();
@@ -194,81 +211,114 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
 
   if (warp < 4) {
     ptx::setmaxnreg_dec<56>();
-    if (warp == 0 && lane == 0) {
+    // Both single-issuer roles run on a WHOLE warp in uniform control flow (every lane walks the
+    // schedule and waits on the barriers); only the TMA / tcgen05 instructions themselves sit under
+    // elect.sync.  A lone `lane == 0` thread would force ptxas to wrap every UTCHMMA / UTMALDG in a
+    // register->uniform-register waterfall loop (measured: ~100 cycles of issue per MMA).
+    auto bcast_segment = [&](Segment g) {
+      g.head = __shfl_sync(0xffffffffu, g.head, 0);
+      g.pair = __shfl_sync(0xffffffffu, g.pair, 0);
+      g.j0 = __shfl_sync(0xffffffffu, g.j0, 0);
+      g.j1 = __shfl_sync(0xffffffffu, g.j1, 0);
+      g.n_tiles = __shfl_sync(0xffffffffu, g.n_tiles, 0);
+      return g;
+    };
+    const int n_cache_tiles = p.n_cache_tiles;
+    if (warp == 0) {
       // ============================== TMA producer ==============================
       uint32_t it = 0, seg = 0;
       auto load_kv = [&](const Segment& g, int j, bool is_v) {
         const uint32_t slot = it % kStages, ph = (it / kStages) & 1;
         ptx::mbar_wait(ptx::smem_u32(&bar.kv_empty[slot]), ph ^ 1);
         const uint32_t full = ptx::smem_u32(&bar.kv_full[slot]);
-        ptx::mbar_arrive_expect_tx(full, C::kTileBytes);
         const uint32_t dst = sKV + slot * C::kTileBytes;
-        if (j < p.n_cache_tiles) {
-          const void* map = is_v ? (const void*)&p.map_vc : (const void*)&p.map_kc;
+        if (ptx::elect_one()) {
+          ptx::mbar_arrive_expect_tx(full, C::kTileBytes);
+          if (j < n_cache_tiles) {
+            const void* map = is_v ? (const void*)&p.map_vc : (const void*)&p.map_kc;
 #pragma unroll
-          for (int a = 0; a < C::kAtoms; ++a) ptx::tma_load_3d(dst + a * C::kAtomBytes, map, full, a * 64, j * kBlockN, g.head);
-        } else {
-          const void* map = is_v ? (const void*)&p.map_vn : (const void*)&p.map_kn;
-          const int r0 = (j - p.n_cache_tiles) * kBlockN;
+            for (int a = 0; a < C::kAtoms; ++a) ptx::tma_load_3d(dst + a * C::kAtomBytes, map, full, a * 64, j * kBlockN, g.head);
+          } else {
+            const void* map = is_v ? (const void*)&p.map_vn : (const void*)&p.map_kn;
+            const int r0 = (j - n_cache_tiles) * kBlockN;
 #pragma unroll
-          for (int a = 0; a < C::kAtoms; ++a) ptx::tma_load_3d(dst + a * C::kAtomBytes, map, full, a * 64, g.head, r0);
+            for (int a = 0; a < C::kAtoms; ++a) ptx::tma_load_3d(dst + a * C::kAtomBytes, map, full, a * 64, g.head, r0);
+          }
         }
+        __syncwarp();
         ++it;
       };
       for (int64_t t = t_lo; t < t_hi; ++seg) {
-        const Segment g = next_segment(sched, p, t, t_hi);
+        const Segment g = bcast_segment(next_segment(sched, p, t, t_hi));
         ptx::mbar_wait(ptx::smem_u32(&bar.q_empty), (seg & 1) ^ 1);
         const uint32_t qf = ptx::smem_u32(&bar.q_full);
-        ptx::mbar_arrive_expect_tx(qf, 2 * C::kTileBytes);
+        if (ptx::elect_one()) {
+          ptx::mbar_arrive_expect_tx(qf, 2 * C::kTileBytes);
 #pragma unroll
-        for (int tile = 0; tile < 2; ++tile)
+          for (int tile = 0; tile < 2; ++tile)
 #pragma unroll
-          for (int a = 0; a < C::kAtoms; ++a)
-            ptx::tma_load_3d(sQ + tile * C::kTileBytes + a * C::kAtomBytes, &p.map_q, qf, a * 64, g.head,
-                             g.pair * kPairM + tile * kBlockM);
+            for (int a = 0; a < C::kAtoms; ++a)
+              ptx::tma_load_3d(sQ + tile * C::kTileBytes + a * C::kAtomBytes, &p.map_q, qf, a * 64, g.head,
+                               g.pair * kPairM + tile * kBlockM);
+        }
+        __syncwarp();
         load_kv(g, g.j0, false);
         for (int j = g.j0; j < g.j1; ++j) {
           load_kv(g, j, true);
           if (j + 1 < g.j1) load_kv(g, j + 1, false);
         }
       }
-    } else if (warp == 1 && lane == 0) {
+    } else if (warp == 1) {
       // ============================== MMA issuer ==============================
       uint32_t it = 0, seg = 0, p_phase = 0;
-      const uint32_t tS[2] = {tmem + C::kTmemS0, tmem + C::kTmemS1};
-      const uint32_t tO[2] = {tmem + C::kTmemO0, tmem + C::kTmemO1};
+      WS_TRACE_DECL(0, lane == 0)
+      const uint32_t tmem_u = __shfl_sync(0xffffffffu, tmem, 0);
+      // K-major SW128 operand (Q, K): LBO 16 B, SBO 1024 B; MN-major SW128 operand (V): LBO = atom, SBO 1024 B
+      constexpr uint64_t kDescK = ((uint64_t)(16 >> 4) << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
+      constexpr uint64_t kDescV = ((uint64_t)(C::kAtomBytes >> 4) << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
+      const uint64_t dQ = kDescK | (uint64_t)((sQ & 0x3FFFFu) >> 4);
+      const uint64_t dKV = (uint64_t)((sKV & 0x3FFFFu) >> 4);
+      // S(tile) = Q(tile) . K(slot)^T
       auto issue_qk = [&](int tile, uint32_t slot) {
-        const uint32_t qa = sQ + tile * C::kTileBytes, kb = sKV + slot * C::kTileBytes;
+        const uint64_t qa = dQ + (uint64_t)(tile * (C::kTileBytes >> 4));
+        const uint64_t kb = (kDescK | dKV) + (uint64_t)(slot * (C::kTileBytes >> 4));
+        const uint32_t ts = tmem_u + (tile ? C::kTmemS1 : C::kTmemS0);
 #pragma unroll
         for (int k = 0; k < D / 16; ++k) {
-          const uint32_t off = (k >> 2) * C::kAtomBytes + (k & 3) * 32;
-          ptx::mma_ss(tS[tile], ptx::make_sdesc_sw128(qa + off, 16, 1024), ptx::make_sdesc_sw128(kb + off, 16, 1024),
-                      C::kIdescQK, k > 0);
+          const uint32_t off = ((k >> 2) * C::kAtomBytes + (k & 3) * 32) >> 4;
+          ptx::mma_ss(ts, qa + off, kb + off, C::kIdescQK, k > 0);
         }
       };
-      auto issue_pv = [&](int tile, uint32_t slot, bool acc) {
-        const uint32_t vb = sKV + slot * C::kTileBytes;
+      // O(tile) (+)= P(tile)[:, 64*half .. 64*half+64) . V(slot)[64*half .. , :]
+      auto issue_pv = [&](int tile, uint32_t slot, int half, bool acc) {
+        const uint64_t vb = (kDescV | dKV) + (uint64_t)(slot * (C::kTileBytes >> 4));
+        const uint32_t ts = tmem_u + (tile ? C::kTmemS1 : C::kTmemS0);
+        const uint32_t to = tmem_u + (tile ? C::kTmemO1 : C::kTmemO0);
 #pragma unroll
-        for (int k = 0; k < kBlockN / 16; ++k)
-          ptx::mma_ts(tO[tile], tS[tile] + k * 8, ptx::make_sdesc_sw128(vb + k * 2048, C::kAtomBytes, 1024), C::kIdescPV,
-                      acc || k > 0);
+        for (int kk = 0; kk < kBlockN / 32; ++kk) {
+          const int k = half * (kBlockN / 32) + kk;
+          ptx::mma_ts(to, ts + k * 8, vb + (uint64_t)(k * (2048 >> 4)), C::kIdescPV, acc || k > 0);
+        }
       };
       auto wait_full = [&](uint32_t i) {
         ptx::mbar_wait(ptx::smem_u32(&bar.kv_full[i % kStages]), (i / kStages) & 1);
         ptx::tc_fence_after();
       };
       for (int64_t t = t_lo; t < t_hi; ++seg) {
-        const Segment g = next_segment(sched, p, t, t_hi);
+        const Segment g = bcast_segment(next_segment(sched, p, t, t_hi));
         ptx::mbar_wait(ptx::smem_u32(&bar.q_full), seg & 1);
         wait_full(it);
         {
           const uint32_t slot = it % kStages;
-          issue_qk(0, slot);
-          ptx::tc_commit(ptx::smem_u32(&bar.s_full[0]));
-          issue_qk(1, slot);
-          ptx::tc_commit(ptx::smem_u32(&bar.s_full[1]));
-          ptx::tc_commit(ptx::smem_u32(&bar.kv_empty[slot]));
-          if (g.j0 + 1 == g.j1) ptx::tc_commit(ptx::smem_u32(&bar.q_empty));
+          if (ptx::elect_one()) {
+            issue_qk(0, slot);
+            ptx::tc_commit(ptx::smem_u32(&bar.s_full[0]));
+            issue_qk(1, slot);
+            ptx::tc_commit(ptx::smem_u32(&bar.s_full[1]));
+            ptx::tc_commit(ptx::smem_u32(&bar.kv_empty[slot]));
+            if (g.j0 + 1 == g.j1) ptx::tc_commit(ptx::smem_u32(&bar.q_empty));
+          }
+          __syncwarp();
           ++it;
         }
         for (int j = g.j0; j < g.j1; ++j) {
@@ -277,25 +327,33 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
           uint32_t it_k = 0, slot_k = 0;
           if (has_next) { it_k = it++; slot_k = it_k % kStages; }
           wait_full(it_v);
-          ptx::mbar_wait(ptx::smem_u32(&bar.p_full[0]), p_phase);
-          ptx::tc_fence_after();
-          issue_pv(0, slot_v, acc);
-          ptx::tc_commit(ptx::smem_u32(&bar.o_done[0]));
-          if (has_next) {
-            wait_full(it_k);
-            issue_qk(0, slot_k);
-            ptx::tc_commit(ptx::smem_u32(&bar.s_full[0]));
-          }
-          ptx::mbar_wait(ptx::smem_u32(&bar.p_full[1]), p_phase);
-          ptx::tc_fence_after();
-          issue_pv(1, slot_v, acc);
-          ptx::tc_commit(ptx::smem_u32(&bar.o_done[1]));
-          ptx::tc_commit(ptx::smem_u32(&bar.kv_empty[slot_v]));
-          if (has_next) {
-            issue_qk(1, slot_k);
-            ptx::tc_commit(ptx::smem_u32(&bar.s_full[1]));
-            ptx::tc_commit(ptx::smem_u32(&bar.kv_empty[slot_k]));
-            if (j + 2 == g.j1) ptx::tc_commit(ptx::smem_u32(&bar.q_empty));
+          WS_TRACE(1);
+#pragma unroll
+          for (int tile = 0; tile < 2; ++tile) {
+            ptx::mbar_wait(ptx::smem_u32(&bar.p_lo[tile]), p_phase);
+            ptx::tc_fence_after();
+            WS_TRACE(2 + 4 * tile);
+            if (ptx::elect_one()) issue_pv(tile, slot_v, 0, acc);
+            __syncwarp();
+            ptx::mbar_wait(ptx::smem_u32(&bar.p_hi[tile]), p_phase);
+            ptx::tc_fence_after();
+            if (tile == 0 && has_next) wait_full(it_k);
+            WS_TRACE(3 + 4 * tile);
+            if (ptx::elect_one()) {
+              issue_pv(tile, slot_v, 1, acc);
+              ptx::tc_commit(ptx::smem_u32(&bar.o_done[tile]));
+              if (tile == 1) ptx::tc_commit(ptx::smem_u32(&bar.kv_empty[slot_v]));
+              if (has_next) {
+                issue_qk(tile, slot_k);
+                ptx::tc_commit(ptx::smem_u32(&bar.s_full[tile]));
+                if (tile == 1) {
+                  ptx::tc_commit(ptx::smem_u32(&bar.kv_empty[slot_k]));
+                  if (j + 2 == g.j1) ptx::tc_commit(ptx::smem_u32(&bar.q_empty));
+                }
+              }
+            }
+            __syncwarp();
+            WS_TRACE(4 + 4 * tile);
           }
           p_phase ^= 1;
         }
@@ -309,8 +367,10 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
     const uint32_t lane_off = (uint32_t)((warp & 3) << 5) << 16;
     const uint32_t tS = tmem + (tile ? C::kTmemS1 : C::kTmemS0) + lane_off;
     const uint32_t tO = tmem + (tile ? C::kTmemO1 : C::kTmemO0) + lane_off;
-    const uint32_t s_full = ptx::smem_u32(&bar.s_full[tile]), p_full = ptx::smem_u32(&bar.p_full[tile]);
+    const uint32_t s_full = ptx::smem_u32(&bar.s_full[tile]);
+    const uint32_t p_lo = ptx::smem_u32(&bar.p_lo[tile]), p_hi = ptx::smem_u32(&bar.p_hi[tile]);
     const uint32_t o_done = ptx::smem_u32(&bar.o_done[tile]);
+    WS_TRACE_DECL(1 + tile, (warp & 3) == 0 && lane == 0)
     uint32_t n_iter = 0;  // S tiles consumed so far == PVs requested so far (drives every phase bit)
 
     for (int64_t t = t_lo; t < t_hi;) {
@@ -328,10 +388,12 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
 
         ptx::mbar_wait(s_full, n_iter & 1);
         ptx::tc_fence_after();
+        WS_TRACE(10);
         uint32_t s[4][32];
 #pragma unroll
         for (int q = 0; q < 4; ++q) ptx::tmem_ld32(tS + q * 32, s[q]);
         ptx::tc_wait_ld();
+        WS_TRACE(11);
         if (lim < kBlockN) {
 #pragma unroll
           for (int q = 0; q < 4; ++q)
@@ -339,11 +401,18 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
             for (int c = 0; c < 32; ++c)
               if (q * 32 + c >= lim) s[q][c] = 0xff800000u;  // -inf
         }
-        float mx = __uint_as_float(s[0][0]);
+        // row maximum: 8 independent chains (a single chain is latency-bound: 64 dependent FMNMX3)
+        float mx8[8];
+#pragma unroll
+        for (int a = 0; a < 8; ++a) mx8[a] = __uint_as_float(s[0][a]);
 #pragma unroll
         for (int q = 0; q < 4; ++q)
 #pragma unroll
-          for (int c = 0; c < 32; ++c) mx = fmaxf(mx, __uint_as_float(s[q][c]));
+          for (int c = (q == 0 ? 8 : 0); c < 32; c += 16)
+#pragma unroll
+            for (int a = 0; a < 8; ++a)
+              mx8[a] = fmaxf(mx8[a], fmaxf(__uint_as_float(s[q][c + a]), __uint_as_float(s[q][(c + 8 + a) & 31])));
+        const float mx = fmaxf(fmaxf(fmaxf(mx8[0], mx8[1]), fmaxf(mx8[2], mx8[3])), fmaxf(fmaxf(mx8[4], mx8[5]), fmaxf(mx8[6], mx8[7])));
         const float m_new = fmaxf(m, mx);
         const bool grow = (m_new - m) * p.scale_log2 > kRescaleThreshold;  // false when both are -inf (NaN)
         if (j == g.j0) {
@@ -365,24 +434,39 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
           }
         }
         const float neg_ms = (m == -INFINITY) ? 0.f : -m * p.scale_log2;
-        uint32_t pk[2][32];
-        float sum0 = 0.f, sum1 = 0.f;
+        WS_TRACE(12);
+        // P = 2^(s*scale - m*scale) in two halves of 64 keys; each half is handed to the MMA warp as soon
+        // as it sits in TMEM, so P.V of the first half overlaps the exponentials of the second.
+        // Tiles in which some row of this warp has masked keys take the all-MUFU variant: ex2(-inf) is
+        // exactly 0 there, while the polynomial clamps to 2^-126 (an empty row must sum to l == 0, R11).
+        const float2 sc2 = make_float2(p.scale_log2, p.scale_log2), nm2 = make_float2(neg_ms, neg_ms);
+        float2 sumA = make_float2(0.f, 0.f), sumB = make_float2(0.f, 0.f);
+        auto exp_halves = [&](auto poly_tag) {
+          constexpr int kPoly = decltype(poly_tag)::value;
 #pragma unroll
-        for (int q = 0; q < 4; ++q)
+          for (int half = 0; half < 2; ++half) {
+            uint32_t pk[32];
 #pragma unroll
-          for (int c = 0; c < 32; c += 2) {
-            const float p0 = ptx::ex2(fmaf(__uint_as_float(s[q][c]), p.scale_log2, neg_ms));
-            const float p1 = ptx::ex2(fmaf(__uint_as_float(s[q][c + 1]), p.scale_log2, neg_ms));
-            sum0 += p0;
-            sum1 += p1;
-            pk[q >> 1][((q & 1) << 4) | (c >> 1)] = ptx::pack_bf16(p0, p1);
+            for (int i = 0; i < 32; ++i) {
+              const int q = half * 2 + (i >> 4), c = (i & 15) * 2;
+              const float2 x = ptx::fma2(make_float2(__uint_as_float(s[q][c]), __uint_as_float(s[q][c + 1])), sc2, nm2);
+              float2 e;
+              if ((i & 3) < kPoly) e = ptx::ex2_poly2(x);
+              else e = make_float2(ptx::ex2(x.x), ptx::ex2(x.y));
+              if (i & 1) sumB = ptx::add2(sumB, e); else sumA = ptx::add2(sumA, e);
+              pk[i] = ptx::pack_bf16(e.x, e.y);
+            }
+            ptx::tmem_st32(tS + half * 32, pk);
+            ptx::tc_wait_st();
+            ptx::tc_fence_before();
+            ptx::mbar_arrive(half ? p_hi : p_lo);
+            WS_TRACE(13 + half);
           }
-        l += sum0 + sum1;
-        ptx::tmem_st32(tS, pk[0]);
-        ptx::tmem_st32(tS + 32, pk[1]);
-        ptx::tc_wait_st();
-        ptx::tc_fence_before();
-        ptx::mbar_arrive(p_full);
+        };
+        if (__any_sync(0xffffffffu, lim < kBlockN)) exp_halves(std::integral_constant<int, 0>{});
+        else exp_halves(std::integral_constant<int, kPolyOf4>{});
+        const float2 sum2 = ptx::add2(sumA, sumB);
+        l += sum2.x + sum2.y;
       }
 
       // ------------------------------ segment epilogue ------------------------------
@@ -605,6 +689,13 @@ int launch_attention(const Params& prm, int64_t total_iters, cudaStream_t stream
 }
 
 }  // namespace
+
+#ifdef WS_ATTN_TRACE
+extern "C" __attribute__((visibility("default"))) void ws_debug_set_trace(void* p) {
+  unsigned long long* v = reinterpret_cast<unsigned long long*>(p);
+  cudaMemcpyToSymbol(g_trace_ptr, &v, sizeof(v));
+}
+#endif
 
 extern "C" __attribute__((visibility("default"))) size_t ws_block_causal_attn_workspace_bytes(int32_t Lq, int32_t H, int32_t d, int64_t kv_total, ws_dtype dt) {
   if (Lq <= 0 || H <= 0 || d <= 0 || kv_total < 0) return 0;

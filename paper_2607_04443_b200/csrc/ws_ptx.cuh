@@ -158,6 +158,39 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
   return r;
 }
 
+// ------------------------------------------------------------------ packed FP32 pairs (sm_100 FFMA2 / FADD2)
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
+// a + b rounded toward -inf, both halves
+__device__ __forceinline__ float2 add2_rm(float2 a, float2 b) {
+  uint64_t ra, rb, rd;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(ra) : "f"(a.x), "f"(a.y));
+  asm("mov.b64 %0, {%1, %2};" : "=l"(rb) : "f"(b.x), "f"(b.y));
+  asm("add.rm.ftz.f32x2 %0, %1, %2;" : "=l"(rd) : "l"(ra), "l"(rb));
+  float2 d;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(d.x), "=f"(d.y) : "l"(rd));
+  return d;
+}
+// 2^x for a pair on the FMA/ALU pipes (no MUFU): Cody-Waite split x = n + f, f in [0,1), degree-3
+// minimax polynomial for 2^f (max relative error 7.5e-5, below BF16's 2^-9), exponent spliced in
+// with an integer add.  Valid for x in [-126, 126]; the caller's values are <= 2^8 by construction
+// and -inf (masked) is clamped to -126 (2^-126: contributes nothing).
+__device__ __forceinline__ float2 ex2_poly2(float2 x) {
+  const float kMagic = 12582912.f;  // 1.5 * 2^23: ulp 1 => x + kMagic (round down) holds floor(x) in its low mantissa bits
+  x.x = fmaxf(x.x, -126.f);
+  x.y = fmaxf(x.y, -126.f);
+  const float2 xr = add2_rm(x, make_float2(kMagic, kMagic));
+  const float2 nf = add2(xr, make_float2(-kMagic, -kMagic));
+  const float2 f = add2(x, make_float2(-nf.x, -nf.y));
+  float2 p = fma2(f, make_float2(0.07802452f, 0.07802452f), make_float2(0.22606716f, 0.22606716f));
+  p = fma2(p, f, make_float2(0.69583356f, 0.69583356f));
+  p = fma2(p, f, make_float2(0.9999252f, 0.9999252f));
+  float2 r;
+  r.x = __uint_as_float(__float_as_uint(p.x) + (__float_as_uint(xr.x) << 23));
+  r.y = __uint_as_float(__float_as_uint(p.y) + (__float_as_uint(xr.y) << 23));
+  return r;
+}
+
 template <int N>
 __device__ __forceinline__ void setmaxnreg_inc() {
   asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N));
