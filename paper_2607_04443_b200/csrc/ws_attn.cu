@@ -29,9 +29,13 @@
 
 #ifdef WS_ATTN_TRACE
 __device__ unsigned long long* g_trace_ptr = nullptr;
-#define WS_TRACE_DECL(role, cond) unsigned long long* trc_ = (blockIdx.x == 5 && g_trace_ptr && (cond)) ? g_trace_ptr + (role) * 8192 : nullptr; int trc_i_ = 0;
+#define WS_TRACE_DECL(role, cond) unsigned long long* trc_ = (blockIdx.x == WS_TRACE_BLOCK && g_trace_ptr && (cond)) ? g_trace_ptr + (role) * 8192 : nullptr; int trc_i_ = 0;
 #define WS_TRACE(ev) do { if (trc_ && trc_i_ < 8190) trc_[trc_i_++] = ((unsigned long long)(ev) << 48) | ((unsigned long long)clock64() & 0xffffffffffffull); } while (0)
+#define WS_TRACE_CTA(slot, ev) do { if (g_trace_ptr && threadIdx.x == (slot) * 32) { unsigned long long gt_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt_)); g_trace_ptr[4 * 8192 + blockIdx.x * 8 + (ev)] = gt_; if ((ev) == 0) { unsigned sm_; asm volatile("mov.u32 %0, %%smid;" : "=r"(sm_)); g_trace_ptr[4 * 8192 + blockIdx.x * 8 + 6] = sm_; } } } while (0)
+#define WS_TRACE_GT(ev) do { if (trc_ && trc_i_ < 8190) { unsigned long long gt_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt_)); trc_[trc_i_++] = ((unsigned long long)(ev) << 48) | (gt_ & 0xffffffffffffull); } } while (0)
 #else
+#define WS_TRACE_GT(ev)
+#define WS_TRACE_CTA(slot, ev)
 #define WS_TRACE_DECL(role, cond)
 #define WS_TRACE(ev)
 #endif
@@ -42,6 +46,7 @@ constexpr int kBlockM = 128;  // query rows per tile (one TMEM lane each)
 constexpr int kBlockN = 128;  // keys per tile
 constexpr int kPairM = 2 * kBlockM;
 constexpr int kStages = 5;    // K/V ring slots
+constexpr int kPChunks = 4;   // P is handed to the MMA warp in chunks of kBlockN / kPChunks keys
 constexpr int kThreads = 384; // warp 0 TMA, warp 1 MMA, warp 2 TMEM alloc, warp 3 idle, warps 4-7 / 8-11 softmax
 constexpr int kMaxPairs = 256;
 constexpr int kMaxCtas = 256; // upper bound on the persistent grid (workspace sizing)
@@ -65,10 +70,7 @@ struct alignas(64) Params {
   float scale, scale_log2;
   int32_t q_block_end[WS_MAX_MASK_BLOCKS];
   int32_t kv_visible[WS_MAX_MASK_BLOCKS];
-};
-
-struct Sched {
-  int32_t pair_prefix[kMaxPairs + 1];  // KV-tile iterations before pair p (per head)
+  int32_t pair_prefix[kMaxPairs + 1];  // KV-tile iterations before Q-tile pair p (per head); host-built schedule
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -84,27 +86,7 @@ __device__ __forceinline__ int block_of_row(const Params& p, int row) {
   return lo;
 }
 
-__device__ __forceinline__ int tiles_for(const Params& p, int nvis) {
-  if (nvis <= 0) return 0;
-  if ((int64_t)nvis <= p.cache_len) return (nvis + kBlockN - 1) / kBlockN;
-  return p.n_cache_tiles + (int)((nvis - p.cache_len + kBlockN - 1) / kBlockN);
-}
-
-// All threads of the CTA call this; ends with __syncthreads().
-__device__ void build_sched(const Params& p, Sched& s) {
-  for (int pr = threadIdx.x; pr < p.n_pairs; pr += blockDim.x) {
-    const int last_row = min((pr + 1) * kPairM, p.Lq) - 1;
-    s.pair_prefix[pr + 1] = tiles_for(p, p.kv_visible[block_of_row(p, last_row)]);
-  }
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    s.pair_prefix[0] = 0;
-    for (int pr = 0; pr < p.n_pairs; ++pr) s.pair_prefix[pr + 1] += s.pair_prefix[pr];
-  }
-  __syncthreads();
-}
-
-__device__ __forceinline__ int pair_of_iter(const Sched& s, int n_pairs, int rem) {
+__device__ __forceinline__ int pair_of_iter(const Params& s, int n_pairs, int rem) {
   int lo = 0, hi = n_pairs - 1;  // largest p with pair_prefix[p] <= rem
   while (lo < hi) {
     const int mid = (lo + hi + 1) >> 1;
@@ -121,7 +103,8 @@ struct Segment {
 };
 
 // Walks the CTA's share [t, hi) of the flattened iteration space.
-__device__ __forceinline__ Segment next_segment(const Sched& s, const Params& p, int64_t& t, int64_t hi) {
+__device__ __forceinline__ Segment next_segment(const Params& p, int64_t& t, int64_t hi) {
+  const Params& s = p;
   const int Tp = s.pair_prefix[p.n_pairs];
   Segment g;
   g.head = (int)(t / Tp);
@@ -145,7 +128,8 @@ struct Cfg {
   static constexpr int kTileBytes = kAtoms * kAtomBytes;  // one Q tile == one K or V tile
   static constexpr int kSmemQ = 2 * kTileBytes;
   static constexpr int kSmemKV = kStages * kTileBytes;
-  static constexpr int kSmemBytes = 1024 /*align slack*/ + kSmemQ + kSmemKV + 256 /*barriers*/ + (int)sizeof(Sched);
+  static constexpr int kSmemBytes = kSmemQ + kSmemKV + 256 /*barriers*/;
+  static_assert(kSmemBytes <= 227 * 1024, "shared memory budget");
   static constexpr uint32_t kTmemS0 = 0, kTmemS1 = 128, kTmemO0 = 256, kTmemO1 = 256 + D;
   static constexpr uint32_t kIdescQK = ptx::make_idesc_bf16(kBlockM, kBlockN, false);
   static constexpr uint32_t kIdescPV = ptx::make_idesc_bf16(kBlockM, D, true);
@@ -154,26 +138,27 @@ struct Cfg {
 struct Barriers {
   uint64_t kv_full[kStages], kv_empty[kStages];
   uint64_t q_full, q_empty;
-  uint64_t s_full[2], p_lo[2], p_hi[2], o_done[2];  // p_lo / p_hi: P of keys [0,64) / [64,128) is in TMEM
+  uint64_t s_full[2], p_ready[2][kPChunks], o_done[2];  // p_ready[t][c]: P of keys [32c, 32c+32) of tile t is in TMEM
   uint32_t tmem_base;
 };
 
 template <int D, bool OUT_F32>
 __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_constant__ Params p) {
   using C = Cfg<D>;
-  extern __shared__ uint8_t smem_raw[];
   // 1024-byte alignment is required by the 128-byte swizzle (TMA box and UMMA descriptor agree on it)
-  const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;
-  uint8_t* smem = smem_raw + (smem_base - ptx::smem_u32(smem_raw));
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  const uint32_t smem_base = ptx::smem_u32(smem_raw);
+  if ((smem_base & 1023u) != 0) __trap();
+  uint8_t* smem = smem_raw;
   const uint32_t sQ = smem_base;
   const uint32_t sKV = smem_base + C::kSmemQ;
   Barriers& bar = *reinterpret_cast<Barriers*>(smem + C::kSmemQ + C::kSmemKV);
-  Sched& sched = *reinterpret_cast<Sched*>(smem + C::kSmemQ + C::kSmemKV + 256);
   static_assert(sizeof(Barriers) <= 256, "barrier block");
 
   // the warp index goes through a shuffle so that ptxas knows it is warp-uniform: the TMA and MMA
   // warps then run in uniform control flow and their descriptors live in uniform registers
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
+  WS_TRACE_CTA(0, 0);
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < kStages; ++i) {
@@ -184,8 +169,7 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
     ptx::mbar_init(ptx::smem_u32(&bar.q_empty), 1);
     for (int t = 0; t < 2; ++t) {
       ptx::mbar_init(ptx::smem_u32(&bar.s_full[t]), 1);
-      ptx::mbar_init(ptx::smem_u32(&bar.p_lo[t]), kBlockM);
-      ptx::mbar_init(ptx::smem_u32(&bar.p_hi[t]), kBlockM);
+      for (int c = 0; c < kPChunks; ++c) ptx::mbar_init(ptx::smem_u32(&bar.p_ready[t][c]), kBlockM);
       ptx::mbar_init(ptx::smem_u32(&bar.o_done[t]), 1);
     }
     ptx::fence_mbar_init();
@@ -199,13 +183,14 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
     ptx::tmem_alloc(ptx::smem_u32(&bar.tmem_base), kTmemCols);
     ptx::tmem_relinquish();
   }
-  build_sched(p, sched);  // includes __syncthreads()
+  __syncthreads();
   ptx::tc_fence_before();
   __syncthreads();
   ptx::tc_fence_after();
   const uint32_t tmem = bar.tmem_base;
+  WS_TRACE_CTA(0, 1);
 
-  const int Tp = sched.pair_prefix[p.n_pairs];
+  const int Tp = p.pair_prefix[p.n_pairs];
   const int64_t T = (int64_t)Tp * p.H;
   const int64_t t_lo = cta_begin(blockIdx.x, T, gridDim.x), t_hi = cta_begin(blockIdx.x + 1, T, gridDim.x);
 
@@ -249,7 +234,7 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
         ++it;
       };
       for (int64_t t = t_lo; t < t_hi; ++seg) {
-        const Segment g = bcast_segment(next_segment(sched, p, t, t_hi));
+        const Segment g = bcast_segment(next_segment(p, t, t_hi));
         ptx::mbar_wait(ptx::smem_u32(&bar.q_empty), (seg & 1) ^ 1);
         const uint32_t qf = ptx::smem_u32(&bar.q_full);
         if (ptx::elect_one()) {
@@ -272,6 +257,8 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
       // ============================== MMA issuer ==============================
       uint32_t it = 0, seg = 0, p_phase = 0;
       WS_TRACE_DECL(0, lane == 0)
+      WS_TRACE(30); WS_TRACE_GT(31);
+      WS_TRACE_CTA(1, 2);
       const uint32_t tmem_u = __shfl_sync(0xffffffffu, tmem, 0);
       // K-major SW128 operand (Q, K): LBO 16 B, SBO 1024 B; MN-major SW128 operand (V): LBO = atom, SBO 1024 B
       constexpr uint64_t kDescK = ((uint64_t)(16 >> 4) << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
@@ -289,14 +276,14 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
           ptx::mma_ss(ts, qa + off, kb + off, C::kIdescQK, k > 0);
         }
       };
-      // O(tile) (+)= P(tile)[:, 64*half .. 64*half+64) . V(slot)[64*half .. , :]
-      auto issue_pv = [&](int tile, uint32_t slot, int half, bool acc) {
+      // O(tile) (+)= P(tile)[:, 32*chunk .. 32*chunk+32) . V(slot)[32*chunk .. , :]
+      auto issue_pv = [&](int tile, uint32_t slot, int chunk, bool acc) {
         const uint64_t vb = (kDescV | dKV) + (uint64_t)(slot * (C::kTileBytes >> 4));
         const uint32_t ts = tmem_u + (tile ? C::kTmemS1 : C::kTmemS0);
         const uint32_t to = tmem_u + (tile ? C::kTmemO1 : C::kTmemO0);
 #pragma unroll
-        for (int kk = 0; kk < kBlockN / 32; ++kk) {
-          const int k = half * (kBlockN / 32) + kk;
+        for (int kk = 0; kk < kBlockN / 16 / kPChunks; ++kk) {
+          const int k = chunk * (kBlockN / 16 / kPChunks) + kk;
           ptx::mma_ts(to, ts + k * 8, vb + (uint64_t)(k * (2048 >> 4)), C::kIdescPV, acc || k > 0);
         }
       };
@@ -305,7 +292,7 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
         ptx::tc_fence_after();
       };
       for (int64_t t = t_lo; t < t_hi; ++seg) {
-        const Segment g = bcast_segment(next_segment(sched, p, t, t_hi));
+        const Segment g = bcast_segment(next_segment(p, t, t_hi));
         ptx::mbar_wait(ptx::smem_u32(&bar.q_full), seg & 1);
         wait_full(it);
         {
@@ -330,17 +317,20 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
           WS_TRACE(1);
 #pragma unroll
           for (int tile = 0; tile < 2; ++tile) {
-            ptx::mbar_wait(ptx::smem_u32(&bar.p_lo[tile]), p_phase);
-            ptx::tc_fence_after();
-            WS_TRACE(2 + 4 * tile);
-            if (ptx::elect_one()) issue_pv(tile, slot_v, 0, acc);
-            __syncwarp();
-            ptx::mbar_wait(ptx::smem_u32(&bar.p_hi[tile]), p_phase);
+#pragma unroll
+            for (int c = 0; c + 1 < kPChunks; ++c) {
+              ptx::mbar_wait(ptx::smem_u32(&bar.p_ready[tile][c]), p_phase);
+              ptx::tc_fence_after();
+              if (c == 0) WS_TRACE(2 + 4 * tile);
+              if (ptx::elect_one()) issue_pv(tile, slot_v, c, acc);
+              __syncwarp();
+            }
+            ptx::mbar_wait(ptx::smem_u32(&bar.p_ready[tile][kPChunks - 1]), p_phase);
             ptx::tc_fence_after();
             if (tile == 0 && has_next) wait_full(it_k);
             WS_TRACE(3 + 4 * tile);
             if (ptx::elect_one()) {
-              issue_pv(tile, slot_v, 1, acc);
+              issue_pv(tile, slot_v, kPChunks - 1, acc);
               ptx::tc_commit(ptx::smem_u32(&bar.o_done[tile]));
               if (tile == 1) ptx::tc_commit(ptx::smem_u32(&bar.kv_empty[slot_v]));
               if (has_next) {
@@ -358,6 +348,8 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
           p_phase ^= 1;
         }
       }
+      WS_TRACE(32); WS_TRACE_GT(33);
+      WS_TRACE_CTA(1, 3);
     }
   } else {
     // ============================== softmax warpgroups ==============================
@@ -368,16 +360,18 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
     const uint32_t tS = tmem + (tile ? C::kTmemS1 : C::kTmemS0) + lane_off;
     const uint32_t tO = tmem + (tile ? C::kTmemO1 : C::kTmemO0) + lane_off;
     const uint32_t s_full = ptx::smem_u32(&bar.s_full[tile]);
-    const uint32_t p_lo = ptx::smem_u32(&bar.p_lo[tile]), p_hi = ptx::smem_u32(&bar.p_hi[tile]);
+    const uint32_t p_ready = ptx::smem_u32(&bar.p_ready[tile][0]);
     const uint32_t o_done = ptx::smem_u32(&bar.o_done[tile]);
     WS_TRACE_DECL(1 + tile, (warp & 3) == 0 && lane == 0)
     uint32_t n_iter = 0;  // S tiles consumed so far == PVs requested so far (drives every phase bit)
 
     for (int64_t t = t_lo; t < t_hi;) {
-      const Segment g = next_segment(sched, p, t, t_hi);
+      const Segment g = next_segment(p, t, t_hi);
       const int row = g.pair * kPairM + tile * kBlockM + row_in_tile;
       const bool row_valid = row < p.Lq;
-      const int nvis = row_valid ? p.kv_visible[block_of_row(p, row)] : 0;
+      // padding rows (>= Lq; their Q is TMA zero fill, their output is never stored) see what the last real row
+      // sees: masking them would push their whole warp onto the slower boundary path for every tile
+      const int nvis = p.kv_visible[block_of_row(p, min(row, p.Lq - 1))];
       const int vis_cache = (int)min((int64_t)nvis, p.cache_len);
       float m = -INFINITY, l = 0.f;  // running max in raw-score units, running sum
 
@@ -435,32 +429,32 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
         }
         const float neg_ms = (m == -INFINITY) ? 0.f : -m * p.scale_log2;
         WS_TRACE(12);
-        // P = 2^(s*scale - m*scale) in two halves of 64 keys; each half is handed to the MMA warp as soon
-        // as it sits in TMEM, so P.V of the first half overlaps the exponentials of the second.
+        // P = 2^(s*scale - m*scale) in kPChunks chunks of 32 keys; each chunk is handed to the MMA warp as soon
+        // as it sits in TMEM, so that P.V of the early chunks overlaps the exponentials of the later ones.
         // Tiles in which some row of this warp has masked keys take the all-MUFU variant: ex2(-inf) is
         // exactly 0 there, while the polynomial clamps to 2^-126 (an empty row must sum to l == 0, R11).
         const float2 sc2 = make_float2(p.scale_log2, p.scale_log2), nm2 = make_float2(neg_ms, neg_ms);
         float2 sumA = make_float2(0.f, 0.f), sumB = make_float2(0.f, 0.f);
         auto exp_halves = [&](auto poly_tag) {
           constexpr int kPoly = decltype(poly_tag)::value;
+          static_assert(kPChunks == 4, "one 32-column TMEM load per chunk");
 #pragma unroll
-          for (int half = 0; half < 2; ++half) {
-            uint32_t pk[32];
+          for (int q = 0; q < kPChunks; ++q) {
+            uint32_t pk[16];
 #pragma unroll
-            for (int i = 0; i < 32; ++i) {
-              const int q = half * 2 + (i >> 4), c = (i & 15) * 2;
-              const float2 x = ptx::fma2(make_float2(__uint_as_float(s[q][c]), __uint_as_float(s[q][c + 1])), sc2, nm2);
+            for (int i = 0; i < 16; ++i) {
+              const float2 x = ptx::fma2(make_float2(__uint_as_float(s[q][2 * i]), __uint_as_float(s[q][2 * i + 1])), sc2, nm2);
               float2 e;
               if ((i & 3) < kPoly) e = ptx::ex2_poly2(x);
               else e = make_float2(ptx::ex2(x.x), ptx::ex2(x.y));
               if (i & 1) sumB = ptx::add2(sumB, e); else sumA = ptx::add2(sumA, e);
               pk[i] = ptx::pack_bf16(e.x, e.y);
             }
-            ptx::tmem_st32(tS + half * 32, pk);
+            ptx::tmem_st16(tS + q * 16, pk);
             ptx::tc_wait_st();
             ptx::tc_fence_before();
-            ptx::mbar_arrive(half ? p_hi : p_lo);
-            WS_TRACE(13 + half);
+            ptx::mbar_arrive(p_ready + q * 8);
+            if (q == 1 || q == 3) WS_TRACE(13 + (q >> 1));
           }
         };
         if (__any_sync(0xffffffffu, lim < kBlockN)) exp_halves(std::integral_constant<int, 0>{});
@@ -526,7 +520,9 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
   }
 
   ptx::tc_fence_before();
+  WS_TRACE_CTA(4, 4);
   __syncthreads();
+  WS_TRACE_CTA(0, 5);
   if (warp == 2) ptx::tmem_dealloc(tmem, kTmemCols);
 }
 
@@ -536,19 +532,17 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
 // ---------------------------------------------------------------------------------------------
 template <int D, bool OUT_F32>
 __global__ void __launch_bounds__(kPairM) attn_combine_kernel(const __grid_constant__ Params p, int attn_grid) {
-  __shared__ Sched sched;
-  build_sched(p, sched);
   const int w = blockIdx.y, head = w / p.n_pairs, pair = w - head * p.n_pairs;
   const int q4 = blockIdx.x, r = threadIdx.x;
   const int row = pair * kPairM + r;
   if (row >= p.Lq) return;
-  const int Tp = sched.pair_prefix[p.n_pairs];
-  const int n_tiles = sched.pair_prefix[pair + 1] - sched.pair_prefix[pair];
+  const int Tp = p.pair_prefix[p.n_pairs];
+  const int n_tiles = p.pair_prefix[pair + 1] - p.pair_prefix[pair];
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
   float lse = -INFINITY;
   if (n_tiles > 0) {
     const int64_t T = (int64_t)Tp * p.H;
-    const int64_t a = (int64_t)head * Tp + sched.pair_prefix[pair];
+    const int64_t a = (int64_t)head * Tp + p.pair_prefix[pair];
     const int c_lo = cta_of_iter(a, T, attn_grid), c_hi = cta_of_iter(a + n_tiles - 1, T, attn_grid);
     if (c_lo == c_hi) return;  // one CTA covered the whole KV range and wrote the final rows itself
     float M = -INFINITY;
@@ -717,7 +711,7 @@ extern "C" __attribute__((visibility("default"))) int ws_block_causal_attn(void*
   if (cache_len > 0 && (!k_cache || !v_cache)) return WS_ERR_INVALID_ARG;
   if (mask->n_blocks <= 0 || !mask->q_block_end || !mask->kv_visible) return WS_ERR_INVALID_ARG;
   if (mask->n_blocks > WS_MAX_MASK_BLOCKS) return WS_ERR_UNSUPPORTED;
-  if (cache_len + Ln > 0x7fffffffLL - kBlockN) return WS_ERR_UNSUPPORTED;
+  if (cache_len + Ln > 0x7fffffffLL / kMaxPairs - kBlockN) return WS_ERR_UNSUPPORTED;  // pair_prefix is int32
   {
     int32_t prev_end = 0, prev_vis = 0;
     for (int b = 0; b < mask->n_blocks; ++b) {
@@ -790,14 +784,17 @@ extern "C" __attribute__((visibility("default"))) int ws_block_causal_attn(void*
     prm.kv_visible[b] = mask->kv_visible[b];
   }
   // total KV-tile iterations (host copy of the device schedule)
+  // the schedule: a Q-tile pair visits the KV tiles its last row can see
   int64_t Tp = 0;
+  prm.pair_prefix[0] = 0;
   for (int pr = 0; pr < n_pairs; ++pr) {
     const int last_row = ((pr + 1) * kPairM < Lq ? (pr + 1) * kPairM : Lq) - 1;
     int b = 0;
     while (last_row >= mask->q_block_end[b]) ++b;
     const int64_t nvis = mask->kv_visible[b];
-    if (nvis <= 0) continue;
-    Tp += nvis <= cache_len ? (nvis + kBlockN - 1) / kBlockN : prm.n_cache_tiles + (nvis - cache_len + kBlockN - 1) / kBlockN;
+    if (nvis > 0)
+      Tp += nvis <= cache_len ? (nvis + kBlockN - 1) / kBlockN : prm.n_cache_tiles + (nvis - cache_len + kBlockN - 1) / kBlockN;
+    prm.pair_prefix[pr + 1] = (int32_t)Tp;
   }
   if (launches) wsi::count_launch(launches);
   const bool f32 = dt == WS_DTYPE_F32;
