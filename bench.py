@@ -251,14 +251,25 @@ def bandwidth_aux(peaks):
     g = torch.Generator(device="cuda").manual_seed(5)
     rnd = lambda *s: torch.randn(*s, generator=g, device="cuda", dtype=torch.float32).to(torch.bfloat16)
 
-    def time_calls(calls, reps=3):
+    def time_calls(calls, reps=3, graph=False):
+        """Best-of-reps average time per call.  graph=True captures the whole call list in ONE CUDA graph
+        (SURVEY.md 8(d)(i)): the literal-size calls take a few microseconds each, less than the host
+        needs to issue one through ctypes, so eager launches would time the host, not the kernel."""
+        run = lambda: [c() for c in calls]
+        if graph:
+            stream = torch.cuda.Stream()
+            cg = torch.cuda.CUDAGraph()
+            torch.cuda.synchronize()
+            with torch.cuda.graph(cg, stream=stream):
+                run()
+            run = cg.replay
+            run()
         best = None
         for _ in range(reps):
             torch.cuda.synchronize()
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record()
-            for c in calls:
-                c()
+            run()
             b.record()
             torch.cuda.synchronize()
             ms = a.elapsed_time(b) / len(calls)
@@ -271,7 +282,7 @@ def bandwidth_aux(peaks):
     srcs = [(rnd(n, H, d), rnd(n, H, d)) for _ in range(24)]
     calls = [(lambda i=i: ws.kv_cache_write(kc, vc, srcs[i % 24][0], srcs[i % 24][1], 0, (i % 64) * n)) for i in range(192)]
     time_calls(calls[:8], 1)
-    ms = time_calls(calls)
+    ms = time_calls(calls, graph=True)
     byts = 2 * 2 * n * H * d * 2
     res["cache_write_cfg3"] = {"us": ms * 1e3, "gbs": byts / ms / 1e6, "bytes": byts, "frac_hbm": byts / ms / 1e6 / peaks["hbm_gbs"]}
     # a1 saturating variant: one call writing all 65536 rows (1.34 GB payload per tensor pair)
@@ -287,11 +298,11 @@ def bandwidth_aux(peaks):
     dsts = [torch.empty((1, L, H // P, d), dtype=torch.bfloat16, device="cuda") for _ in range(56)]
     calls = [(lambda i=i: ws.seq_to_head(dsts[i % 56], srcs[i % 28], P, i % 4, 1)) for i in range(224)]
     time_calls(calls[:8], 1)
-    ms = time_calls(calls)
+    ms = time_calls(calls, graph=True)
     byts = 2 * L * (H // P) * d * 2
     res["seq_to_head_cfg4"] = {"us": ms * 1e3, "gbs": byts / ms / 1e6, "bytes": byts, "frac_hbm": byts / ms / 1e6 / peaks["hbm_gbs"]}
     calls = [(lambda i=i: ws.head_to_seq(srcs[i % 28], dsts[i % 56], P, i % 4, 1)) for i in range(224)]
-    ms = time_calls(calls)
+    ms = time_calls(calls, graph=True)
     res["head_to_seq_cfg4"] = {"us": ms * 1e3, "gbs": byts / ms / 1e6, "bytes": byts, "frac_hbm": byts / ms / 1e6 / peaks["hbm_gbs"]}
     # saturating variant: G = P full pack of a 32x longer sequence (1.2 GB read + 1.2 GB written)
     Lb = 3680 * 32

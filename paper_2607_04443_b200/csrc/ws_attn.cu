@@ -71,6 +71,13 @@ struct alignas(64) Params {
   int32_t q_block_end[WS_MAX_MASK_BLOCKS];
   int32_t kv_visible[WS_MAX_MASK_BLOCKS];
   int32_t pair_prefix[kMaxPairs + 1];  // KV-tile iterations before Q-tile pair p (per head); host-built schedule
+  // Two-phase schedule (host-built).  Work item i = head * n_pairs + pair.  Phase 1: CTA c runs the whole
+  // items w * grid + c, w < n_waves (no partials; the pairs of one head start together on neighbouring
+  // CTAs, so a K/V tile is fetched from DRAM once and hit in L2 by the other pairs).  Phase 2: the
+  // remaining items [n_waves * grid, H * n_pairs) are split stream-K style, CTA c taking the flattened
+  // KV-tile iterations [pool_begin[c], pool_begin[c + 1]) (global coordinates head * Tp + pair_prefix).
+  int32_t n_waves, grid;
+  int64_t pool_begin[kMaxCtas + 1];
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -95,15 +102,22 @@ __device__ __forceinline__ int pair_of_iter(const Params& s, int n_pairs, int re
   return lo;
 }
 
-__device__ __forceinline__ int64_t cta_begin(int64_t c, int64_t T, int64_t G) { return (c * T) / G; }
-__device__ __forceinline__ int cta_of_iter(int64_t t, int64_t T, int64_t G) { return (int)(((t + 1) * G - 1) / T); }
+// the CTA whose phase-2 range holds flattened iteration t (pool_begin is non-decreasing; empty ranges are skipped)
+__device__ __forceinline__ int cta_of_iter(const Params& p, int64_t t) {
+  int lo = 0, hi = p.grid - 1;  // largest c with pool_begin[c] <= t
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if (p.pool_begin[mid] <= t) lo = mid; else hi = mid - 1;
+  }
+  return lo;
+}
 
 struct Segment {
   int head, pair, j0, j1, n_tiles;  // KV tiles [j0, j1) of the pair's n_tiles
 };
 
-// Walks the CTA's share [t, hi) of the flattened iteration space.
-__device__ __forceinline__ Segment next_segment(const Params& p, int64_t& t, int64_t hi) {
+// Walks the CTA's phase-2 share [t, hi) of the flattened iteration space.
+__device__ __forceinline__ Segment next_pool_segment(const Params& p, int64_t& t, int64_t hi) {
   const Params& s = p;
   const int Tp = s.pair_prefix[p.n_pairs];
   Segment g;
@@ -117,6 +131,33 @@ __device__ __forceinline__ Segment next_segment(const Params& p, int64_t& t, int
   t += g.j1 - g.j0;
   return g;
 }
+
+// A CTA's walk over its segments: whole items first (phase 1), then its stream-K range (phase 2).
+// Every role of the CTA runs the same walk, so they agree on the segment sequence.  An item that
+// sees no key at all is reported with n_tiles == 0 (phase 1 only): the softmax warps zero-fill its
+// rows, the TMA and MMA warps skip it.
+struct SegWalk {
+  int wave;
+  int64_t t, hi;
+  __device__ __forceinline__ SegWalk(const Params& p) : wave(0), t(p.pool_begin[blockIdx.x]), hi(p.pool_begin[blockIdx.x + 1]) {}
+  __device__ __forceinline__ bool next(const Params& p, Segment& g) {
+    if (wave < p.n_waves) {
+      const int item = wave * p.grid + (int)blockIdx.x;
+      ++wave;
+      g.head = item / p.n_pairs;
+      g.pair = item - g.head * p.n_pairs;
+      g.n_tiles = p.pair_prefix[g.pair + 1] - p.pair_prefix[g.pair];
+      g.j0 = 0;
+      g.j1 = g.n_tiles;
+      return true;
+    }
+    if (t < hi) {
+      g = next_pool_segment(p, t, hi);
+      return true;
+    }
+    return false;
+  }
+};
 
 // ---------------------------------------------------------------------------------------------
 // the attention kernel
@@ -190,10 +231,6 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
   const uint32_t tmem = bar.tmem_base;
   WS_TRACE_CTA(0, 1);
 
-  const int Tp = p.pair_prefix[p.n_pairs];
-  const int64_t T = (int64_t)Tp * p.H;
-  const int64_t t_lo = cta_begin(blockIdx.x, T, gridDim.x), t_hi = cta_begin(blockIdx.x + 1, T, gridDim.x);
-
   if (warp < 4) {
     ptx::setmaxnreg_dec<56>();
     // Both single-issuer roles run on a WHOLE warp in uniform control flow (every lane walks the
@@ -233,8 +270,10 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
         __syncwarp();
         ++it;
       };
-      for (int64_t t = t_lo; t < t_hi; ++seg) {
-        const Segment g = bcast_segment(next_segment(p, t, t_hi));
+      SegWalk walk(p);
+      for (Segment g0; walk.next(p, g0);) {
+        const Segment g = bcast_segment(g0);
+        if (g.n_tiles == 0) continue;
         ptx::mbar_wait(ptx::smem_u32(&bar.q_empty), (seg & 1) ^ 1);
         const uint32_t qf = ptx::smem_u32(&bar.q_full);
         if (ptx::elect_one()) {
@@ -252,6 +291,7 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
           load_kv(g, j, true);
           if (j + 1 < g.j1) load_kv(g, j + 1, false);
         }
+        ++seg;
       }
     } else if (warp == 1) {
       // ============================== MMA issuer ==============================
@@ -291,8 +331,10 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
         ptx::mbar_wait(ptx::smem_u32(&bar.kv_full[i % kStages]), (i / kStages) & 1);
         ptx::tc_fence_after();
       };
-      for (int64_t t = t_lo; t < t_hi; ++seg) {
-        const Segment g = bcast_segment(next_segment(p, t, t_hi));
+      SegWalk walk(p);
+      for (Segment g0; walk.next(p, g0);) {
+        const Segment g = bcast_segment(g0);
+        if (g.n_tiles == 0) continue;
         ptx::mbar_wait(ptx::smem_u32(&bar.q_full), seg & 1);
         wait_full(it);
         {
@@ -347,6 +389,7 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
           }
           p_phase ^= 1;
         }
+        ++seg;
       }
       WS_TRACE(32); WS_TRACE_GT(33);
       WS_TRACE_CTA(1, 3);
@@ -365,10 +408,21 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
     WS_TRACE_DECL(1 + tile, (warp & 3) == 0 && lane == 0)
     uint32_t n_iter = 0;  // S tiles consumed so far == PVs requested so far (drives every phase bit)
 
-    for (int64_t t = t_lo; t < t_hi;) {
-      const Segment g = next_segment(p, t, t_hi);
+    SegWalk walk(p);
+    for (Segment g; walk.next(p, g);) {
       const int row = g.pair * kPairM + tile * kBlockM + row_in_tile;
       const bool row_valid = row < p.Lq;
+      if (g.n_tiles == 0) {
+        // no key is visible to this Q-tile pair (reading R11): output rows 0, LSE -inf
+        if (row_valid) {
+          if (p.lse != nullptr) p.lse[(int64_t)g.head * p.Lq + row] = -INFINITY;
+          constexpr int kRowVecs = D * (OUT_F32 ? 4 : 2) / 16;
+          uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<char*>(p.out) + ((int64_t)row * p.H + g.head) * D * (OUT_F32 ? 4 : 2));
+#pragma unroll
+          for (int c = 0; c < kRowVecs; ++c) dst[c] = make_uint4(0u, 0u, 0u, 0u);
+        }
+        continue;
+      }
       // padding rows (>= Lq; their Q is TMA zero fill, their output is never stored) see what the last real row
       // sees: masking them would push their whole warp onto the slower boundary path for every tile
       const int nvis = p.kv_visible[block_of_row(p, min(row, p.Lq - 1))];
@@ -527,12 +581,12 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
 }
 
 // ---------------------------------------------------------------------------------------------
-// combine kernel: merges split-KV partials, and zero-fills Q-pairs that see no key at all.
-// grid = (d/4, H * n_pairs), block = 256 threads (one per row of the pair).
+// combine kernel: merges the split-KV partials of the phase-2 items, and zero-fills phase-2 items
+// that see no key at all.  grid = (d/4, number of phase-2 items), block = 256 threads (one per row).
 // ---------------------------------------------------------------------------------------------
 template <int D, bool OUT_F32>
-__global__ void __launch_bounds__(kPairM) attn_combine_kernel(const __grid_constant__ Params p, int attn_grid) {
-  const int w = blockIdx.y, head = w / p.n_pairs, pair = w - head * p.n_pairs;
+__global__ void __launch_bounds__(kPairM) attn_combine_kernel(const __grid_constant__ Params p) {
+  const int w = p.n_waves * p.grid + blockIdx.y, head = w / p.n_pairs, pair = w - head * p.n_pairs;
   const int q4 = blockIdx.x, r = threadIdx.x;
   const int row = pair * kPairM + r;
   if (row >= p.Lq) return;
@@ -541,9 +595,8 @@ __global__ void __launch_bounds__(kPairM) attn_combine_kernel(const __grid_const
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
   float lse = -INFINITY;
   if (n_tiles > 0) {
-    const int64_t T = (int64_t)Tp * p.H;
     const int64_t a = (int64_t)head * Tp + p.pair_prefix[pair];
-    const int c_lo = cta_of_iter(a, T, attn_grid), c_hi = cta_of_iter(a + n_tiles - 1, T, attn_grid);
+    const int c_lo = cta_of_iter(p, a), c_hi = cta_of_iter(p, a + n_tiles - 1);
     if (c_lo == c_hi) return;  // one CTA covered the whole KV range and wrote the final rows itself
     float M = -INFINITY;
     for (int c = c_lo; c <= c_hi; ++c) M = fmaxf(M, p.part_ml[((int64_t)w + c) * kPairM + r].x);
@@ -659,7 +712,7 @@ WsLayout ws_layout(int32_t Lq, int32_t H, int32_t d, int64_t kv_total, int64_t c
 }
 
 template <int D, bool OUT_F32>
-int launch_attention(const Params& prm, int64_t total_iters, cudaStream_t stream) {
+int launch_attention(const Params& prm, cudaStream_t stream) {
   using C = Cfg<D>;
   static std::once_flag once;
   static cudaError_t attr_err = cudaSuccess;
@@ -669,16 +722,18 @@ int launch_attention(const Params& prm, int64_t total_iters, cudaStream_t stream
   if (attr_err != cudaSuccess) return wsi::cuda_fail(attr_err);
   const int sms = sm_count();
   if (sms <= 0) return wsi::cuda_fail(cudaErrorNoDevice);
-  int grid = (int)(total_iters < (int64_t)sms ? total_iters : (int64_t)sms);
-  if (grid > kMaxCtas) grid = kMaxCtas;
+  (void)sms;
   int launches = 0;
-  if (grid > 0) {
-    attn_fwd_kernel<D, OUT_F32><<<grid, kThreads, C::kSmemBytes, stream>>>(prm);
+  if (prm.grid > 0) {
+    attn_fwd_kernel<D, OUT_F32><<<prm.grid, kThreads, C::kSmemBytes, stream>>>(prm);
     ++launches;
   }
-  dim3 cgrid(D / 4, (unsigned)(prm.H * prm.n_pairs));
-  attn_combine_kernel<D, OUT_F32><<<cgrid, kPairM, 0, stream>>>(prm, grid > 0 ? grid : 1);
-  ++launches;
+  const int n_pool_items = prm.H * prm.n_pairs - prm.n_waves * prm.grid;
+  if (n_pool_items > 0) {
+    dim3 cgrid(D / 4, (unsigned)n_pool_items);
+    attn_combine_kernel<D, OUT_F32><<<cgrid, kPairM, 0, stream>>>(prm);
+    ++launches;
+  }
   return wsi::after_launch(launches);
 }
 
@@ -796,8 +851,54 @@ extern "C" __attribute__((visibility("default"))) int ws_block_causal_attn(void*
       Tp += nvis <= cache_len ? (nvis + kBlockN - 1) / kBlockN : prm.n_cache_tiles + (nvis - cache_len + kBlockN - 1) / kBlockN;
     prm.pair_prefix[pr + 1] = (int32_t)Tp;
   }
+  // ---- two-phase schedule (see Params) ----
+  {
+    const int sms = sm_count();
+    if (sms <= 0) return wsi::cuda_fail(cudaErrorNoDevice);
+    const int64_t T = Tp * H, n_items = (int64_t)H * n_pairs;
+    int64_t G = T > 0 ? T : n_items;
+    if (G > sms) G = sms;
+    if (G > kMaxCtas) G = kMaxCtas;
+    prm.grid = (int32_t)G;
+    auto item_len = [&](int64_t i) { const int pr = (int)(i % n_pairs); return (int64_t)(prm.pair_prefix[pr + 1] - prm.pair_prefix[pr]); };
+    auto item_flat = [&](int64_t i) { return (i / n_pairs) * Tp + prm.pair_prefix[i % n_pairs]; };
+    // candidate B: W whole-item waves, the remaining items water-filled over the CTAs
+    const int64_t W = n_items / G;
+    int64_t p1[kMaxCtas], quota[kMaxCtas];
+    int64_t pool = T, p1_max = 0;
+    for (int64_t c = 0; c < G; ++c) {
+      p1[c] = 0;
+      for (int64_t w = 0; w < W; ++w) p1[c] += item_len(w * G + c);
+      pool -= p1[c];
+      if (p1[c] > p1_max) p1_max = p1[c];
+    }
+    // smallest level with sum_c max(0, level - p1[c]) >= pool
+    int64_t lo = 0, hi = p1_max + pool;
+    while (lo < hi) {
+      const int64_t mid = (lo + hi) / 2;
+      int64_t cap = 0;
+      for (int64_t c = 0; c < G; ++c) cap += mid > p1[c] ? mid - p1[c] : 0;
+      if (cap >= pool) hi = mid; else lo = mid + 1;
+    }
+    int64_t excess = -pool;
+    for (int64_t c = 0; c < G; ++c) { quota[c] = lo > p1[c] ? lo - p1[c] : 0; excess += quota[c]; }
+    for (int64_t c = G - 1; c >= 0 && excess > 0; --c)
+      if (quota[c] > 0) { --quota[c]; --excess; }
+    const int64_t makespan_b = lo > p1_max ? lo : p1_max, makespan_a = (T + G - 1) / G;
+    // B trades a slightly longer critical path for far fewer split items and L2 reuse of K/V across the pairs of a head
+    const bool use_b = W > 0 && makespan_b * 100 <= makespan_a * 103;
+    if (use_b) {
+      prm.n_waves = (int32_t)W;
+      int64_t t = item_flat(W * G);
+      for (int64_t c = 0; c < G; ++c) { prm.pool_begin[c] = t; t += quota[c]; }
+      prm.pool_begin[G] = t;  // == T
+    } else {
+      prm.n_waves = 0;
+      for (int64_t c = 0; c <= G; ++c) prm.pool_begin[c] = (c * T) / G;
+    }
+  }
   if (launches) wsi::count_launch(launches);
   const bool f32 = dt == WS_DTYPE_F32;
-  if (d == 128) return f32 ? launch_attention<128, true>(prm, Tp * H, stream) : launch_attention<128, false>(prm, Tp * H, stream);
-  return f32 ? launch_attention<64, true>(prm, Tp * H, stream) : launch_attention<64, false>(prm, Tp * H, stream);
+  if (d == 128) return f32 ? launch_attention<128, true>(prm, stream) : launch_attention<128, false>(prm, stream);
+  return f32 ? launch_attention<64, true>(prm, stream) : launch_attention<64, false>(prm, stream);
 }
