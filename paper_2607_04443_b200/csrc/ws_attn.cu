@@ -230,6 +230,9 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
   ptx::tc_fence_after();
   const uint32_t tmem = bar.tmem_base;
   WS_TRACE_CTA(0, 1);
+  // everything above touched only shared memory, TMEM and the kernel parameters: it overlaps the previous kernel's tail
+  wsi::pdl_trigger();
+  wsi::pdl_wait();
 
   if (warp < 4) {
     ptx::setmaxnreg_dec<56>();
@@ -586,6 +589,8 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
 // ---------------------------------------------------------------------------------------------
 template <int D, bool OUT_F32>
 __global__ void __launch_bounds__(kPairM) attn_combine_kernel(const __grid_constant__ Params p) {
+  wsi::pdl_trigger();
+  wsi::pdl_wait();  // the partials are the attention kernel's
   const int w = p.n_waves * p.grid + blockIdx.y, head = w / p.n_pairs, pair = w - head * p.n_pairs;
   const int q4 = blockIdx.x, r = threadIdx.x;
   const int row = pair * kPairM + r;
@@ -635,6 +640,8 @@ __global__ void __launch_bounds__(kPairM) attn_combine_kernel(const __grid_const
 // Copies `rows` rows of `row_elems` contiguous floats; source rows `src_pitch` floats apart per plane.
 __global__ void cast_f32_to_bf16_kernel(__nv_bfloat16* __restrict__ dst, const float* __restrict__ src, int64_t n_planes,
                                         int64_t plane_elems, int64_t src_plane_pitch) {
+  wsi::pdl_trigger();
+  wsi::pdl_wait();
   const int64_t total = n_planes * plane_elems;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
     const int64_t pl = i / plane_elems, e = i - pl * plane_elems;
@@ -725,13 +732,15 @@ int launch_attention(const Params& prm, cudaStream_t stream) {
   (void)sms;
   int launches = 0;
   if (prm.grid > 0) {
-    attn_fwd_kernel<D, OUT_F32><<<prm.grid, kThreads, C::kSmemBytes, stream>>>(prm);
+    const cudaError_t e = wsi::launch_pdl(attn_fwd_kernel<D, OUT_F32>, dim3(prm.grid), dim3(kThreads), C::kSmemBytes, stream, prm);
+    if (e != cudaSuccess) return wsi::cuda_fail(e);
     ++launches;
   }
   const int n_pool_items = prm.H * prm.n_pairs - prm.n_waves * prm.grid;
   if (n_pool_items > 0) {
     dim3 cgrid(D / 4, (unsigned)n_pool_items);
-    attn_combine_kernel<D, OUT_F32><<<cgrid, kPairM, 0, stream>>>(prm);
+    const cudaError_t e = wsi::launch_pdl(attn_combine_kernel<D, OUT_F32>, cgrid, dim3(kPairM), 0, stream, prm);
+    if (e != cudaSuccess) return wsi::cuda_fail(e);
     ++launches;
   }
   return wsi::after_launch(launches);
@@ -797,8 +806,8 @@ extern "C" __attribute__((visibility("default"))) int ws_block_causal_attn(void*
       const int64_t total = planes * plane_elems;
       if (total == 0) return;
       const int blocks = (int)((total + 255) / 256 < 4096 ? (total + 255) / 256 : 4096);
-      cast_f32_to_bf16_kernel<<<blocks, 256, 0, stream>>>(reinterpret_cast<__nv_bfloat16*>(dstp),
-                                                          reinterpret_cast<const float*>(srcp), planes, plane_elems, pitch);
+      (void)wsi::launch_pdl(cast_f32_to_bf16_kernel, dim3(blocks), dim3(256), 0, stream, reinterpret_cast<__nv_bfloat16*>(dstp),
+                            reinterpret_cast<const float*>(srcp), planes, plane_elems, pitch);
       ++launches;
     };
     cast(ws + L.stage_q, q, 1, (int64_t)Lq * H * d, 0);

@@ -34,6 +34,7 @@ __device__ __forceinline__ uint4 ld_stream(const uint4* p) {
 __global__ void __launch_bounds__(kThreads) strided_copy16_kernel(const uint4* __restrict__ src0, uint4* __restrict__ dst0,
                                                                   const uint4* __restrict__ src1, uint4* __restrict__ dst1,
                                                                   CopyPlan p) {
+  wsi::pdl_trigger();  // the next kernel may be scheduled now; it blocks in its own pdl_wait() until this grid is done
   const uint4* __restrict__ src = blockIdx.z == 0 ? src0 : src1;
   uint4* __restrict__ dst = blockIdx.z == 0 ? dst0 : dst1;
   const int64_t a = blockIdx.y;
@@ -41,7 +42,7 @@ __global__ void __launch_bounds__(kThreads) strided_copy16_kernel(const uint4* _
   dst += a * p.dst_a;
   const uint32_t base = blockIdx.x * (kThreads * kUnroll) + threadIdx.x;
   uint4 v[kUnroll];
-  int64_t doff[kUnroll];
+  int64_t soff[kUnroll], doff[kUnroll];
 #pragma unroll
   for (int u = 0; u < kUnroll; ++u) {
     const uint32_t idx = base + u * kThreads;
@@ -49,10 +50,14 @@ __global__ void __launch_bounds__(kThreads) strided_copy16_kernel(const uint4* _
     if (idx < p.per_a) {
       const uint32_t b = idx / p.dv;
       const uint32_t c = idx - b * p.dv;
-      v[u] = ld_stream(src + (int64_t)b * p.src_b + c);
+      soff[u] = (int64_t)b * p.src_b + c;
       doff[u] = (int64_t)b * p.dst_b + c;
     }
   }
+  wsi::pdl_wait();  // first global access below: the previous kernel on the stream has completed
+#pragma unroll
+  for (int u = 0; u < kUnroll; ++u)
+    if (doff[u] >= 0) v[u] = ld_stream(src + soff[u]);
 #pragma unroll
   for (int u = 0; u < kUnroll; ++u)
     if (doff[u] >= 0) dst[doff[u]] = v[u];
@@ -76,7 +81,8 @@ int launch_copy(const void* s0, void* d0, const void* s1, void* d1, int n_tensor
     const uint4* ps1 = s1 ? reinterpret_cast<const uint4*>(s1) + b0 * src_b : nullptr;
     uint4* pd1 = d1 ? reinterpret_cast<uint4*>(d1) + b0 * dst_b : nullptr;
     dim3 grid((unsigned)((p.per_a + kThreads * kUnroll - 1) / (kThreads * kUnroll)), (unsigned)A, (unsigned)n_tensors);
-    strided_copy16_kernel<<<grid, kThreads, 0, stream>>>(ps0, pd0, ps1, pd1, p);
+    const cudaError_t e = wsi::launch_pdl(strided_copy16_kernel, grid, dim3(kThreads), 0, stream, ps0, pd0, ps1, pd1, p);
+    if (e != cudaSuccess) return wsi::cuda_fail(e);
     ++launches;
   }
   return wsi::after_launch(launches);

@@ -32,4 +32,31 @@ inline int after_launch(int n_launches) {
   return WS_OK;
 }
 
+// ---- programmatic dependent launch (PDL) ----
+// The hot path is a chain of short kernels on one stream (cache write, relayouts, attention, relayout); the
+// kernel-to-kernel gap is of the order of a relayout's whole HBM time.  Every kernel of the library is launched
+// with programmatic stream serialisation: its CTAs may be scheduled while the previous kernel drains, run their
+// address set-up, and block in pdl_wait() -- which returns once the previous kernel has completed and its
+// writes are visible -- before their FIRST global-memory access.  pdl_trigger() lets the next kernel do the same.
+// A successor that is not one of ours (no attribute) is serialised as usual.  Capturable in CUDA graphs.
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+#endif
+
 }  // namespace wsi
