@@ -603,17 +603,30 @@ __global__ void __launch_bounds__(kPairM) attn_combine_kernel(const __grid_const
     const int64_t a = (int64_t)head * Tp + p.pair_prefix[pair];
     const int c_lo = cta_of_iter(p, a), c_hi = cta_of_iter(p, a + n_tiles - 1);
     if (c_lo == c_hi) return;  // one CTA covered the whole KV range and wrote the final rows itself
-    float M = -INFINITY;
-    for (int c = c_lo; c <= c_hi; ++c) M = fmaxf(M, p.part_ml[((int64_t)w + c) * kPairM + r].x);
-    float L = 0.f;
-    if (M > -INFINITY) {
-      for (int c = c_lo; c <= c_hi; ++c) {
-        const int64_t slot = (int64_t)w + c;
-        const float2 ml = p.part_ml[slot * kPairM + r];
-        const float wgt = ptx::ex2(ml.x - M);  // 0 for an all-masked partial (m = -inf)
-        const float4 o = reinterpret_cast<const float4*>(p.part_o)[(slot * (D / 4) + q4) * kPairM + r];
-        acc.x += wgt * o.x; acc.y += wgt * o.y; acc.z += wgt * o.z; acc.w += wgt * o.w;
-        L += wgt * ml.y;
+    // online LSE-weighted merge, four partials per step so that eight independent loads are in flight per thread
+    float M = -INFINITY, L = 0.f;
+    for (int c = c_lo; c <= c_hi; c += 4) {
+      float2 ml[4];
+      float4 o[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int64_t slot = (int64_t)w + min(c + u, c_hi);
+        ml[u] = p.part_ml[slot * kPairM + r];
+        o[u] = reinterpret_cast<const float4*>(p.part_o)[(slot * (D / 4) + q4) * kPairM + r];
+        if (c + u > c_hi) ml[u] = make_float2(-INFINITY, 0.f);
+      }
+      const float M_new = fmaxf(fmaxf(M, fmaxf(ml[0].x, ml[1].x)), fmaxf(ml[2].x, ml[3].x));
+      if (M_new > -INFINITY) {
+        const float f = ptx::ex2(M - M_new);  // 0 while nothing has been merged yet (M = -inf)
+        acc.x *= f; acc.y *= f; acc.z *= f; acc.w *= f;
+        L *= f;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const float wgt = ptx::ex2(ml[u].x - M_new);  // 0 for an all-masked partial (m = -inf)
+          acc.x += wgt * o[u].x; acc.y += wgt * o[u].y; acc.z += wgt * o[u].z; acc.w += wgt * o[u].w;
+          L += wgt * ml[u].y;
+        }
+        M = M_new;
       }
     }
     if (L > 0.f) {

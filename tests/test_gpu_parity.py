@@ -220,6 +220,10 @@ SHAPES = [
     (7, 1, 128, [50, 50], [0, 64], 64, 0),                 # first block sees nothing
     (8, 5, 64, [700], [2500], 1900, 600),                  # d = 64 multi-tile with split-KV
     (9, 1, 128, [512], [40000], 39500, 500),               # long KV, few Q tiles: deep split-KV + combine
+    # more (head, Q-pair) work items than SMs: whole-item waves first, stream-K only on the remainder
+    (10, 40, 128, [1100], [400], 300, 100),                # 200 equal items: one wave + a 52-item pool
+    (11, 160, 64, [256, 300], [0, 450], 200, 250),         # 480 items, three waves; every pair 0 sees no key at all
+    (12, 30, 128, [256] * 6, [300, 600, 900, 1200, 1500, 1800], 1500, 300),  # 180 items of very unequal length
 ]
 
 
