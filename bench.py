@@ -362,6 +362,36 @@ def attention_aux(peaks):
         ms = a.elapsed_time(b) / reps
         tf = cfg.attn_flops() / ms / 1e9
         res[name] = {"attention_ms": ms, "tflops": tf, "frac_bf16_peak": tf / peaks["bf16_tflops"]}
+        if name == "cfg4":
+            # one Ulysses rank's local step (P = 4): seq->head x3 + attention + head->seq, against the same step
+            # with the relayouts fused into the attention call (strided TMA on the token-major tensors)
+            P, Ht = cfg.P, cfg.H * cfg.P
+            qs, kns, vns = rnd(1.0, L, Ht, d), rnd(cfg.kv_std, L, Ht, d), rnd(cfg.kv_std, L, Ht, d)
+            outs = torch.empty_like(qs)
+            packed = [torch.empty((1, L, H, d), dtype=torch.bfloat16, device="cuda") for _ in range(4)]
+
+            def unfused():
+                for dst, src in zip(packed[:3], (qs, kns, vns)):
+                    ws.seq_to_head(dst, src, P, cfg.g0, 1)
+                ws.block_causal_attn(packed[3][0], packed[0][0], kc, vc, cfg.cache_len, packed[1][0], packed[2][0], cfg.q_block_end,
+                                     cfg.kv_visible, cfg.softmax_scale, wsp)
+                ws.head_to_seq(outs, packed[3], P, cfg.g0, 1)
+
+            def fused():
+                ws.block_causal_attn_seq_layout(outs, qs, kc, vc, cfg.cache_len, kns, vns, cfg.g0 * H, cfg.q_block_end,
+                                                cfg.kv_visible, cfg.softmax_scale, wsp)
+
+            for label, fn in (("unfused", unfused), ("fused", fused)):
+                for _ in range(3):
+                    fn()
+                torch.cuda.synchronize()
+                a.record()
+                for _ in range(reps):
+                    fn()
+                b.record()
+                torch.cuda.synchronize()
+                res[f"cfg4_rank_step_{label}"] = {"ms": a.elapsed_time(b) / reps, "launches": 6 if label == "unfused" else 2}
+            del qs, kns, vns, outs, packed
         if name == "cfg5":
             ks, vs = rnd(cfg.kv_std, cfg.write_rows, H, d), rnd(cfg.kv_std, cfg.write_rows, H, d)
             qs = [rnd(1.0, L, H, d) for _ in range(cfg.steps)]

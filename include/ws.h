@@ -134,6 +134,33 @@ int ws_block_causal_attn(void* out, float* lse, const void* q, const void* k_cac
                          void* workspace, size_t workspace_bytes, ws_dtype dt, void* stream);
 
 /* ------------------------------------------------------------------------------------------------
+ * a2 + a3 + a4 fused: attention straight on the token-major layout
+ *
+ *   The collectives "around attention" exist to hand a rank the full sequence of its own heads.
+ *   When that sequence already sits in local memory as token-major [n_tok, H_total, d] tensors
+ *   (single GPU; or after a peer has written its tokens in place), the two relayouts are pure
+ *   address arithmetic: this call reads the heads [head_begin, head_begin + H) of q_seq,
+ *   k_new_seq, v_new_seq through strided TMA descriptors and stores O into the same heads of
+ *   out_seq, whose other heads are not touched.  It equals
+ *       ws_seq_to_head(q, k_new, v_new) -> ws_block_causal_attn -> ws_head_to_seq(out)
+ *   with P = H_total / H, g0 = head_begin / H, G = 1, bit for bit, without the 4 x n_tok x H x d
+ *   element round trip through HBM.
+ *
+ *   out_seq            : device, [Lq, H_total, d]
+ *   q_seq              : device, [Lq, H_total, d]
+ *   k_new_seq, v_new_seq : device, [Ln, H_total, d]; NULL iff Ln == 0
+ *   k_cache, v_cache   : device, [H, capacity, d]  (the rank's head-sharded cache, as in a3)
+ *   lse                : device, float [H, Lq] (local head index), or NULL
+ *   Everything else as ws_block_causal_attn; workspace size = ..._workspace_bytes(Lq, H, d, ...).
+ *   Errors: as a3, plus INVALID_ARG if head_begin < 0 or head_begin + H > H_total.
+ * ---------------------------------------------------------------------------------------------- */
+int ws_block_causal_attn_seq_layout(void* out_seq, float* lse, const void* q_seq, const void* k_cache,
+                                    const void* v_cache, int64_t capacity, int64_t cache_len, const void* k_new_seq,
+                                    const void* v_new_seq, int32_t Ln, int32_t H_total, int32_t head_begin, int32_t H,
+                                    int32_t d, int32_t Lq, const ws_block_mask* mask, float softmax_scale,
+                                    void* workspace, size_t workspace_bytes, ws_dtype dt, void* stream);
+
+/* ------------------------------------------------------------------------------------------------
  * a5. One unit end to end from HOST buffers ("receive the current K/V slice, update
  *     their local shards of the full-history cache, and run ... denoising for the next unit").
  *

@@ -21,7 +21,7 @@ _lib = None
 
 EXPORTS = (
     "ws_kv_cache_write", "ws_seq_to_head", "ws_head_to_seq", "ws_block_causal_attn_workspace_bytes",
-    "ws_block_causal_attn", "ws_unit_forward_host_staging_bytes", "ws_unit_forward_host", "ws_status_string",
+    "ws_block_causal_attn", "ws_block_causal_attn_seq_layout", "ws_unit_forward_host_staging_bytes", "ws_unit_forward_host", "ws_status_string",
     "ws_version", "ws_last_cuda_error", "ws_kernel_launch_count",
 )
 
@@ -64,6 +64,9 @@ def load():
     lib.ws_block_causal_attn.argtypes = [vp, vp, vp, vp, vp, i64, i64, vp, vp, i32, i32, i32, i32,
                                          ctypes.POINTER(_BlockMask), f32, vp, sz, ctypes.c_int, vp]
     lib.ws_block_causal_attn.restype = ctypes.c_int
+    lib.ws_block_causal_attn_seq_layout.argtypes = [vp, vp, vp, vp, vp, i64, i64, vp, vp, i32, i32, i32, i32, i32, i32,
+                                                    ctypes.POINTER(_BlockMask), f32, vp, sz, ctypes.c_int, vp]
+    lib.ws_block_causal_attn_seq_layout.restype = ctypes.c_int
     lib.ws_unit_forward_host_staging_bytes.argtypes = [i32, i32, i32, i32, i32, i64, i32]
     lib.ws_unit_forward_host_staging_bytes.restype = sz
     lib.ws_unit_forward_host.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp, i64, vp, vp, i32, i64, i64, i32, i32, f32,
@@ -192,6 +195,39 @@ def block_causal_attn(out, q, k_cache, v_cache, cache_len: int, k_new, v_new, q_
                                      _p(v_new), Ln, H, d, Lq, ctypes.byref(mask), float(softmax_scale), _p(workspace),
                                      workspace.numel() * workspace.element_size(), _dt(q), _stream(stream))
     _ok(rc, "ws_block_causal_attn")
+
+
+def block_causal_attn_seq_layout(out_seq, q_seq, k_cache, v_cache, cache_len: int, k_new_seq, v_new_seq, head_begin: int,
+                                 q_block_end: Sequence[int], kv_visible: Sequence[int], softmax_scale: float, workspace,
+                                 lse=None, stream=None):
+    """Relayouts fused into attention (ws.h a2+a3+a4): q_seq/out_seq [Lq, H_total, d], k_new_seq/v_new_seq
+    [Ln, H_total, d] or None; the cache [H, capacity, d] names the H heads [head_begin, head_begin + H) taken."""
+    _dev(out_seq, q_seq, k_cache, v_cache, k_new_seq, v_new_seq, workspace, lse)
+    Lq, H_total, d = q_seq.shape
+    H, capacity = k_cache.shape[0], k_cache.shape[1]
+    Ln = 0 if k_new_seq is None else k_new_seq.shape[0]
+    if out_seq.shape != q_seq.shape or out_seq.dtype != q_seq.dtype:
+        raise ValueError("ws_block_causal_attn_seq_layout: out_seq must match q_seq")
+    if tuple(k_cache.shape) != (H, capacity, d) or v_cache.shape != k_cache.shape:
+        raise ValueError("ws_block_causal_attn_seq_layout: cache must be [H, capacity, d]")
+    if k_new_seq is not None and (tuple(k_new_seq.shape) != (Ln, H_total, d) or v_new_seq is None or v_new_seq.shape != k_new_seq.shape):
+        raise ValueError("ws_block_causal_attn_seq_layout: k_new_seq/v_new_seq must be [Ln, H_total, d]")
+    for t in (k_cache, v_cache, k_new_seq, v_new_seq):
+        if t is not None and t.dtype != q_seq.dtype:
+            raise TypeError("ws_block_causal_attn_seq_layout: dtype mismatch")
+    if lse is not None and (lse.dtype != torch.float32 or tuple(lse.shape) != (H, Lq)):
+        raise ValueError("ws_block_causal_attn_seq_layout: lse must be float32 [H, Lq]")
+    n = len(q_block_end)
+    if len(kv_visible) != n:
+        raise ValueError("ws_block_causal_attn_seq_layout: mask arrays differ in length")
+    qe = (ctypes.c_int32 * n)(*[int(x) for x in q_block_end])
+    kv = (ctypes.c_int32 * n)(*[int(x) for x in kv_visible])
+    mask = _BlockMask(n, qe, kv)
+    rc = load().ws_block_causal_attn_seq_layout(_p(out_seq), _p(lse), _p(q_seq), _p(k_cache), _p(v_cache), capacity, int(cache_len),
+                                                _p(k_new_seq), _p(v_new_seq), Ln, H_total, int(head_begin), H, d, Lq,
+                                                ctypes.byref(mask), float(softmax_scale), _p(workspace),
+                                                workspace.numel() * workspace.element_size(), _dt(q_seq), _stream(stream))
+    _ok(rc, "ws_block_causal_attn_seq_layout")
 
 
 def unit_forward_host_staging_bytes(Lq, Ln, H, d, n_slice_rows, kv_total, n_steps) -> int:

@@ -66,6 +66,7 @@ struct alignas(64) Params {
   float* part_o;   // [slots][d/4][256][4]
   float2* part_ml; // [slots][256] (m * scale * log2e, l)
   int64_t cache_len;
+  int64_t out_pitch;  // elements between consecutive tokens of `out` (H * d, or H_total * d for the token-major rank view)
   int32_t Lq, H, Ln, n_blocks, n_pairs, n_cache_tiles;
   float scale, scale_log2;
   int32_t q_block_end[WS_MAX_MASK_BLOCKS];
@@ -420,7 +421,7 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
         if (row_valid) {
           if (p.lse != nullptr) p.lse[(int64_t)g.head * p.Lq + row] = -INFINITY;
           constexpr int kRowVecs = D * (OUT_F32 ? 4 : 2) / 16;
-          uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<char*>(p.out) + ((int64_t)row * p.H + g.head) * D * (OUT_F32 ? 4 : 2));
+          uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<char*>(p.out) + ((int64_t)row * p.out_pitch + (int64_t)g.head * D) * (OUT_F32 ? 4 : 2));
 #pragma unroll
           for (int c = 0; c < kRowVecs; ++c) dst[c] = make_uint4(0u, 0u, 0u, 0u);
         }
@@ -535,13 +536,13 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
           ptx::tc_wait_ld();
           if (row_valid) {
             if constexpr (OUT_F32) {
-              float4* dst = reinterpret_cast<float4*>(reinterpret_cast<float*>(p.out) + ((int64_t)row * p.H + g.head) * D + ch * 32);
+              float4* dst = reinterpret_cast<float4*>(reinterpret_cast<float*>(p.out) + ((int64_t)row * p.out_pitch + (int64_t)g.head * D) + ch * 32);
 #pragma unroll
               for (int c = 0; c < 8; ++c)
                 dst[c] = make_float4(__uint_as_float(o[4 * c]) * inv, __uint_as_float(o[4 * c + 1]) * inv,
                                      __uint_as_float(o[4 * c + 2]) * inv, __uint_as_float(o[4 * c + 3]) * inv);
             } else {
-              uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<__nv_bfloat16*>(p.out) + ((int64_t)row * p.H + g.head) * D + ch * 32);
+              uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<__nv_bfloat16*>(p.out) + ((int64_t)row * p.out_pitch + (int64_t)g.head * D) + ch * 32);
 #pragma unroll
               for (int c = 0; c < 4; ++c) {
                 uint4 v;
@@ -637,7 +638,7 @@ __global__ void __launch_bounds__(kPairM) attn_combine_kernel(const __grid_const
       acc = make_float4(0.f, 0.f, 0.f, 0.f);
     }
   }
-  const int64_t o_off = ((int64_t)row * p.H + head) * D + q4 * 4;
+  const int64_t o_off = ((int64_t)row * p.out_pitch + (int64_t)head * D) + q4 * 4;
   if constexpr (OUT_F32) {
     *reinterpret_cast<float4*>(reinterpret_cast<float*>(p.out) + o_off) = acc;
   } else {
@@ -773,10 +774,13 @@ extern "C" __attribute__((visibility("default"))) size_t ws_block_causal_attn_wo
   return ws_layout(Lq, H, d, kv_total, 0, 0, dt, false).total;
 }
 
-extern "C" __attribute__((visibility("default"))) int ws_block_causal_attn(void* out, float* lse, const void* q, const void* k_cache, const void* v_cache,
-                                    int64_t capacity, int64_t cache_len, const void* k_new, const void* v_new, int32_t Ln,
-                                    int32_t H, int32_t d, int32_t Lq, const ws_block_mask* mask, float softmax_scale,
-                                    void* workspace, size_t workspace_bytes, ws_dtype dt, void* stream_) {
+namespace {
+// Shared implementation.  q / k_new / v_new / out are token-major with `tok_heads` heads per token in memory, of which
+// the H heads starting at the given base pointers take part (tok_heads == H for the plain [L, H, d] call).
+int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const void* v_cache, int64_t capacity,
+              int64_t cache_len, const void* k_new, const void* v_new, int32_t Ln, int32_t H, int32_t d, int32_t Lq,
+              const ws_block_mask* mask, float softmax_scale, void* workspace, size_t workspace_bytes, ws_dtype dt,
+              void* stream_, int64_t tok_heads) {
   cudaStream_t stream = (cudaStream_t)stream_;
   // ---- validation: nothing is launched on any error ----
   if (dt != WS_DTYPE_BF16 && dt != WS_DTYPE_F32) return WS_ERR_UNSUPPORTED;
@@ -823,11 +827,11 @@ extern "C" __attribute__((visibility("default"))) int ws_block_causal_attn(void*
                             reinterpret_cast<const float*>(srcp), planes, plane_elems, pitch);
       ++launches;
     };
-    cast(ws + L.stage_q, q, 1, (int64_t)Lq * H * d, 0);
+    cast(ws + L.stage_q, q, Lq, (int64_t)H * d, tok_heads * d);  // token by token: the staged copy is compact [Lq, H, d]
     cast(ws + L.stage_kc, k_cache, H, cache_len * d, capacity * d);
     cast(ws + L.stage_vc, v_cache, H, cache_len * d, capacity * d);
-    cast(ws + L.stage_kn, k_new, 1, (int64_t)Ln * H * d, 0);
-    cast(ws + L.stage_vn, v_new, 1, (int64_t)Ln * H * d, 0);
+    cast(ws + L.stage_kn, k_new, Ln, (int64_t)H * d, tok_heads * d);
+    cast(ws + L.stage_vn, v_new, Ln, (int64_t)H * d, tok_heads * d);
     q_b = ws + L.stage_q; kc_b = ws + L.stage_kc; vc_b = ws + L.stage_vc; kn_b = ws + L.stage_kn; vn_b = ws + L.stage_vn;
     cap_b = cache_len;
   }
@@ -835,18 +839,20 @@ extern "C" __attribute__((visibility("default"))) int ws_block_causal_attn(void*
   Params prm;
   memset(&prm, 0, sizeof(prm));
   const uint64_t row_b = (uint64_t)d * 2;
-  bool ok = encode_map(&prm.map_q, q_b, d, H, Lq, row_b, row_b * H, 1, kBlockM);
+  const uint64_t tok_b = row_b * (uint64_t)(dt == WS_DTYPE_F32 ? H : tok_heads);  // token pitch of the BF16 operands
+  bool ok = encode_map(&prm.map_q, q_b, d, H, Lq, row_b, tok_b, 1, kBlockM);
   // a source with no rows still needs a well-formed (never dereferenced) descriptor
-  ok = ok && (Ln > 0 ? encode_map(&prm.map_kn, kn_b, d, H, Ln, row_b, row_b * H, 1, kBlockN)
-                     : encode_map(&prm.map_kn, q_b, d, H, Lq, row_b, row_b * H, 1, kBlockN));
-  ok = ok && (Ln > 0 ? encode_map(&prm.map_vn, vn_b, d, H, Ln, row_b, row_b * H, 1, kBlockN)
-                     : encode_map(&prm.map_vn, q_b, d, H, Lq, row_b, row_b * H, 1, kBlockN));
+  ok = ok && (Ln > 0 ? encode_map(&prm.map_kn, kn_b, d, H, Ln, row_b, tok_b, 1, kBlockN)
+                     : encode_map(&prm.map_kn, q_b, d, H, Lq, row_b, tok_b, 1, kBlockN));
+  ok = ok && (Ln > 0 ? encode_map(&prm.map_vn, vn_b, d, H, Ln, row_b, tok_b, 1, kBlockN)
+                     : encode_map(&prm.map_vn, q_b, d, H, Lq, row_b, tok_b, 1, kBlockN));
   ok = ok && (cache_len > 0 ? encode_map(&prm.map_kc, kc_b, d, cache_len, H, row_b, row_b * cap_b, kBlockN, 1)
-                            : encode_map(&prm.map_kc, q_b, d, H, Lq, row_b, row_b * H, 1, kBlockN));
+                            : encode_map(&prm.map_kc, q_b, d, H, Lq, row_b, tok_b, 1, kBlockN));
   ok = ok && (cache_len > 0 ? encode_map(&prm.map_vc, vc_b, d, cache_len, H, row_b, row_b * cap_b, kBlockN, 1)
-                            : encode_map(&prm.map_vc, q_b, d, H, Lq, row_b, row_b * H, 1, kBlockN));
+                            : encode_map(&prm.map_vc, q_b, d, H, Lq, row_b, tok_b, 1, kBlockN));
   if (!ok) return wsi::cuda_fail(cudaErrorInvalidValue);
   prm.out = out;
+  prm.out_pitch = tok_heads * d;
   prm.lse = lse;
   prm.part_o = reinterpret_cast<float*>(ws + L.part_o);
   prm.part_ml = reinterpret_cast<float2*>(ws + L.part_ml);
@@ -923,4 +929,29 @@ extern "C" __attribute__((visibility("default"))) int ws_block_causal_attn(void*
   const bool f32 = dt == WS_DTYPE_F32;
   if (d == 128) return f32 ? launch_attention<128, true>(prm, stream) : launch_attention<128, false>(prm, stream);
   return f32 ? launch_attention<64, true>(prm, stream) : launch_attention<64, false>(prm, stream);
+}
+}  // namespace
+
+extern "C" __attribute__((visibility("default"))) int ws_block_causal_attn(void* out, float* lse, const void* q, const void* k_cache, const void* v_cache,
+                                    int64_t capacity, int64_t cache_len, const void* k_new, const void* v_new, int32_t Ln,
+                                    int32_t H, int32_t d, int32_t Lq, const ws_block_mask* mask, float softmax_scale,
+                                    void* workspace, size_t workspace_bytes, ws_dtype dt, void* stream) {
+  return attn_impl(out, lse, q, k_cache, v_cache, capacity, cache_len, k_new, v_new, Ln, H, d, Lq, mask, softmax_scale, workspace,
+                   workspace_bytes, dt, stream, H);
+}
+
+// a2 + a3 + a4 in one call: the rank's heads [head_begin, head_begin + H) are read straight from
+// the token-major [n_tok, H_total, d] tensors by strided TMA and O is stored straight back into that layout.
+extern "C" __attribute__((visibility("default"))) int ws_block_causal_attn_seq_layout(void* out_seq, float* lse, const void* q_seq, const void* k_cache,
+                                               const void* v_cache, int64_t capacity, int64_t cache_len, const void* k_new_seq,
+                                               const void* v_new_seq, int32_t Ln, int32_t H_total, int32_t head_begin, int32_t H,
+                                               int32_t d, int32_t Lq, const ws_block_mask* mask, float softmax_scale,
+                                               void* workspace, size_t workspace_bytes, ws_dtype dt, void* stream) {
+  if (dt != WS_DTYPE_BF16 && dt != WS_DTYPE_F32) return WS_ERR_UNSUPPORTED;
+  if (H_total <= 0 || H <= 0 || d <= 0 || head_begin < 0 || (int64_t)head_begin + H > H_total) return WS_ERR_INVALID_ARG;
+  const int64_t off = (int64_t)head_begin * d * wsi::elem_bytes(dt);
+  auto shift = [off](const void* p) { return p ? static_cast<const void*>(static_cast<const char*>(p) + off) : nullptr; };
+  return attn_impl(out_seq ? static_cast<char*>(out_seq) + off : nullptr, lse, shift(q_seq), k_cache, v_cache, capacity, cache_len,
+                   shift(k_new_seq), shift(v_new_seq), Ln, H, d, Lq, mask, softmax_scale, workspace, workspace_bytes, dt, stream,
+                   H_total);
 }

@@ -173,6 +173,61 @@ def test_config_whole_tensor_parity(name):
         check_attn(to_host(out), ref, lse.cpu().numpy(), ref_lse, what=f"{name} step {step}")
 
 
+@pytest.mark.parametrize("name,g0", [("cfg4_small", 0), ("cfg4_small", 3), ("cfg4", 1)])
+def test_relayouts_fused_into_attention(name, g0):
+    """ws_block_causal_attn_seq_layout (a2 + a3 + a4 in one call) on the token-major [L, H_total, d] tensors:
+    bit-identical to seq->head x3 + attention + head->seq through the library, heads of other ranks untouched,
+    and within tolerance of the oracle's composition of the same three definitions."""
+    cfg = wl.CONFIGS[name]
+    x = wl.generate(cfg)
+    dt = cfg.dtype
+    P, Hp, H_total = cfg.P, cfg.H, cfg.H * cfg.P
+    kc, vc = to_dev(x["k_cache"], dt), to_dev(x["v_cache"], dt)
+    q, kn, vn = to_dev(x["q"][0], dt), to_dev(x["k_new"][0], dt), to_dev(x["v_new"][0], dt)
+    assert tuple(q.shape) == (cfg.Lq, H_total, cfg.d)
+    wsp = workspace_for(cfg.Lq, Hp, cfg.d, cfg.cache_len + cfg.Ln, q.dtype)
+    # unfused: three packs, attention, unpack into a sentinel-filled token-major tensor
+    def relay(t):
+        o = torch.empty((1, t.shape[0], Hp, cfg.d), dtype=t.dtype, device="cuda")
+        ws.seq_to_head(o, t, P, g0, 1)
+        return o[0]
+    out_h = torch.empty((cfg.Lq, Hp, cfg.d), dtype=q.dtype, device="cuda")
+    lse_a = torch.empty((Hp, cfg.Lq), dtype=torch.float32, device="cuda")
+    ws.block_causal_attn(out_h, relay(q), kc, vc, cfg.cache_len, relay(kn), relay(vn), cfg.q_block_end, cfg.kv_visible,
+                         cfg.softmax_scale, wsp, lse=lse_a)
+    sentinel = 1.0 / 64.0
+    out_a = torch.full_like(q, sentinel)
+    ws.head_to_seq(out_a, out_h[None], P, g0, 1)
+    # fused
+    out_b = torch.full_like(q, sentinel)
+    lse_b = torch.empty_like(lse_a)
+    ws.block_causal_attn_seq_layout(out_b, q, kc, vc, cfg.cache_len, kn, vn, g0 * Hp, cfg.q_block_end, cfg.kv_visible,
+                                    cfg.softmax_scale, wsp, lse=lse_b)
+    torch.cuda.synchronize()
+    assert np.array_equal(raw_bytes(out_a), raw_bytes(out_b)), "fused and unfused paths must agree bit for bit"
+    assert torch.equal(lse_a, lse_b)
+    got = to_host(out_b)
+    others = np.ones(H_total, bool)
+    others[g0 * Hp:(g0 + 1) * Hp] = False
+    assert np.all(got[:, others] == sentinel), "heads of other ranks must not be touched"
+    # oracle: definitions composed (relayout -> attention), sampled rows at full size
+    def relay_ref(a):
+        o = np.empty((1, a.shape[0], Hp, cfg.d), np.float32)
+        wsref.seq_to_head(o, a, P, g0, 1)
+        return o[0]
+    rq, rkn, rvn = relay_ref(x["q"][0]), relay_ref(x["k_new"][0]), relay_ref(x["v_new"][0])
+    mine = got[:, g0 * Hp:(g0 + 1) * Hp]
+    if name.endswith("_small"):
+        ref, ref_lse = wsref.block_causal_attn(rq, x["k_cache"], x["v_cache"], cfg.cache_len, rkn, rvn, cfg.q_block_end,
+                                               cfg.kv_visible, cfg.softmax_scale)
+        check_attn(mine, ref, lse_b.cpu().numpy(), ref_lse, what=f"{name} fused g0={g0}")
+    else:
+        rows, heads = wl.sample_pairs(cfg, 256)
+        ref, ref_lse = wsref.block_causal_attn_rows(rq, x["k_cache"], x["v_cache"], cfg.cache_len, rkn, rvn, cfg.q_block_end,
+                                                    cfg.kv_visible, cfg.softmax_scale, rows, heads)
+        check_attn(mine[rows, heads], ref, lse_b.cpu().numpy()[heads, rows], ref_lse, what=f"{name} fused g0={g0} (sampled)")
+
+
 def test_config1_also_in_bf16():
     cfg = wl.CONFIGS["cfg1_split"]
     x = wl.generate(cfg)
