@@ -46,7 +46,31 @@ constexpr int kBlockM = 128;  // query rows per tile (one TMEM lane each)
 constexpr int kBlockN = 128;  // keys per tile
 constexpr int kPairM = 2 * kBlockM;
 constexpr int kStages = 5;    // K/V ring slots
-constexpr int kPChunks = 4;   // P is handed to the MMA warp in chunks of kBlockN / kPChunks keys
+// P is handed to the MMA warp in chunks; chunk c covers the 16-key units [chunk16(c), chunk16(c + 1)) of the tile.
+// WS_CHUNK_ENDS lists the chunk ends as decimal digits (2468 = four chunks of 32 keys; 478 = 64 + 48 + 16 keys; the last digit is 8).
+// A small LAST chunk shortens what follows the final hand-off on the critical path (its P.V, then the next Q.K^T).
+#ifndef WS_CHUNK_ENDS
+#define WS_CHUNK_ENDS 478
+#endif
+__host__ __device__ constexpr int chunk_count() {
+  int n = 0;
+  for (int v = WS_CHUNK_ENDS; v > 0; v /= 10) ++n;
+  return n;
+}
+constexpr int kPChunks = chunk_count();
+__host__ __device__ constexpr int chunk16(int c) {  // first 16-key unit of chunk c; chunk16(kPChunks) == 8
+  if (c == 0) return 0;
+  int v = WS_CHUNK_ENDS;
+  for (int i = kPChunks; i > c; --i) v /= 10;
+  return v % 10;
+}
+// index of the chunk that ends after 16-key unit u (u = 1..8), or -1
+__host__ __device__ constexpr int chunk_ending_at(int u) {
+  for (int c = 1; c <= kPChunks; ++c)
+    if (chunk16(c) == u) return c - 1;
+  return -1;
+}
+static_assert(chunk16(0) == 0 && chunk16(kPChunks) == 8, "chunks cover the 128 keys of a tile");
 constexpr int kThreads = 384; // warp 0 TMA, warp 1 MMA, warp 2 TMEM alloc, warp 3 idle, warps 4-7 / 8-11 softmax
 constexpr int kMaxPairs = 256;
 constexpr int kMaxCtas = 256; // upper bound on the persistent grid (workspace sizing)
@@ -180,7 +204,7 @@ struct Cfg {
 struct Barriers {
   uint64_t kv_full[kStages], kv_empty[kStages];
   uint64_t q_full, q_empty;
-  uint64_t s_full[2], p_ready[2][kPChunks], o_done[2];  // p_ready[t][c]: P of keys [32c, 32c+32) of tile t is in TMEM
+  uint64_t s_full[2], p_ready[2][kPChunks], o_done[2];  // p_ready[t][c]: chunk c of tile t's P is in TMEM
   uint32_t tmem_base;
 };
 
@@ -326,8 +350,7 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
         const uint32_t ts = tmem_u + (tile ? C::kTmemS1 : C::kTmemS0);
         const uint32_t to = tmem_u + (tile ? C::kTmemO1 : C::kTmemO0);
 #pragma unroll
-        for (int kk = 0; kk < kBlockN / 16 / kPChunks; ++kk) {
-          const int k = chunk * (kBlockN / 16 / kPChunks) + kk;
+        for (int k = chunk16(chunk); k < chunk16(chunk + 1); ++k) {
           ptx::mma_ts(to, ts + k * 8, vb + (uint64_t)(k * (2048 >> 4)), C::kIdescPV, acc || k > 0);
         }
       };
@@ -495,24 +518,26 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
         float2 sumA = make_float2(0.f, 0.f), sumB = make_float2(0.f, 0.f);
         auto exp_halves = [&](auto poly_tag) {
           constexpr int kPoly = decltype(poly_tag)::value;
-          static_assert(kPChunks == 4, "one 32-column TMEM load per chunk");
 #pragma unroll
-          for (int q = 0; q < kPChunks; ++q) {
-            uint32_t pk[16];
+          for (int u = 0; u < kBlockN / 16; ++u) {  // 16 keys -> 8 packed BF16 pairs -> 8 TMEM columns
+            uint32_t pk[8];
 #pragma unroll
-            for (int i = 0; i < 16; ++i) {
-              const float2 x = ptx::fma2(make_float2(__uint_as_float(s[q][2 * i]), __uint_as_float(s[q][2 * i + 1])), sc2, nm2);
+            for (int i = 0; i < 8; ++i) {
+              const int key = u * 16 + 2 * i;
+              const float2 x = ptx::fma2(make_float2(__uint_as_float(s[key >> 5][key & 31]), __uint_as_float(s[key >> 5][(key & 31) + 1])), sc2, nm2);
               float2 e;
               if ((i & 3) < kPoly) e = ptx::ex2_poly2(x);
               else e = make_float2(ptx::ex2(x.x), ptx::ex2(x.y));
               if (i & 1) sumB = ptx::add2(sumB, e); else sumA = ptx::add2(sumA, e);
               pk[i] = ptx::pack_bf16(e.x, e.y);
             }
-            ptx::tmem_st16(tS + q * 16, pk);
-            ptx::tc_wait_st();
-            ptx::tc_fence_before();
-            ptx::mbar_arrive(p_ready + q * 8);
-            if (q == 1 || q == 3) WS_TRACE(13 + (q >> 1));
+            ptx::tmem_st8(tS + u * 8, pk);
+            if (chunk_ending_at(u + 1) >= 0) {  // compile-time: the loop is fully unrolled
+              ptx::tc_wait_st();
+              ptx::tc_fence_before();
+              ptx::mbar_arrive(p_ready + chunk_ending_at(u + 1) * 8);
+              if (u == 3 || u == 7) WS_TRACE(13 + (u >> 2));
+            }
           }
         };
         if (__any_sync(0xffffffffu, lim < kBlockN)) exp_halves(std::integral_constant<int, 0>{});
