@@ -165,9 +165,16 @@ int ws_block_causal_attn_seq_layout(void* out_seq, float* lse, const void* q_seq
  *     their local shards of the full-history cache, and run ... denoising for the next unit").
  *
  *   Stream-ordered on `stream`:  H2D copies of the slice and of every step's Q/K_new/V_new ->
- *   ws_kv_cache_write (if n_slice_rows > 0) -> n_steps x ws_block_causal_attn (step s uses
- *   q_host[s], k_new_host[s], v_new_host[s]; the mask is the single block "all Lq rows see
+ *   ws_kv_cache_write (if n_slice_rows > 0) -> n_steps x attention (step s uses q_host[s],
+ *   k_new_host[s], v_new_host[s]; the mask is the single block "all Lq rows see
  *   cache_len_after + Ln keys") -> D2H copy of every step's output into out_host[s].
+ *   The unit is PCIe-bound, so the work is pipelined over four head groups (when H % 4 == 0 and
+ *   H >= 8): a group's inputs travel as 2-D copies on an internal copy stream, its cache write and
+ *   attention (ws_block_causal_attn_seq_layout on the group's heads) start on `stream` as soon as
+ *   they have landed, and its output returns on a second internal stream.  Both helper streams
+ *   (one pair per device, created on first use: the library's only lazily created global state
+ *   besides the driver entry point) start after the work already queued on `stream` and are
+ *   joined back into it, so to the caller the call is ordered on `stream` like any other.
  *   The call does not synchronise; the caller synchronises the stream before reading out_host.
  *
  *   k_cache, v_cache : device [H, capacity, d]      (the persistent local cache)
