@@ -329,6 +329,28 @@ def test_block_causal_equals_independent_prefix_calls():
         prev = e
 
 
+def test_heads_are_independent_so_relayout_commutes_with_attention():
+    """What ws_block_causal_attn_seq_layout relies on: attention acts on each head separately,
+    so seq->head, attention on the rank's heads, head->seq equals slicing those heads out of attention on all heads."""
+    P, g0 = 2, 1
+    p = rand_problem(41, 4, 8, [5, 6], [9, 20], 12, 11)          # H = 4 heads in the token-major tensors
+    H, Hp = 4, 2
+    full, full_lse = run(p)                                       # all heads
+    def pack(a):
+        o = np.empty((1, a.shape[0], Hp, a.shape[2]), a.dtype)
+        wsref.seq_to_head(o, a, P, g0, 1)
+        return o[0]
+    sub = dict(p, q=pack(p["q"]), k_new=pack(p["k_new"]), v_new=pack(p["v_new"]),
+               k_cache=np.ascontiguousarray(p["k_cache"][g0 * Hp:(g0 + 1) * Hp]),
+               v_cache=np.ascontiguousarray(p["v_cache"][g0 * Hp:(g0 + 1) * Hp]))
+    o, l = run(sub)
+    back = np.full(full.shape, -7.0)
+    wsref.head_to_seq(back, o[None], P, g0, 1)
+    np.testing.assert_array_equal(back[:, g0 * Hp:(g0 + 1) * Hp], full[:, g0 * Hp:(g0 + 1) * Hp])
+    np.testing.assert_array_equal(l, full_lse[g0 * Hp:(g0 + 1) * Hp])
+    assert np.all(back[:, :g0 * Hp] == -7.0)                      # other ranks' heads untouched
+
+
 def test_spike_key_at_every_boundary():
     """A key with a +40 logit at index kv_visible[b]-1 must dominate block b; at index kv_visible[b]
     it must have no effect on block b.  Also at the cache/new seam."""
