@@ -538,7 +538,8 @@ def run_reference(args):
     kc, vc = x["k_cache"].copy(), x["v_cache"].copy()
     wsref.kv_cache_write(kc, vc, x["k_slice"], x["v_slice"], 0, cfg.write_offset)
     a = (x["q"][0], kc, vc, cfg.cache_len, x["k_new"][0], x["v_new"][0], cfg.q_block_end, cfg.kv_visible, cfg.softmax_scale)
-    n_rows = 192  # per step: a bounded sample (rows are independent); whole run stays within minutes
+    # per step: a bounded sample (rows are independent), shrunk for long runs so that the whole arm stays within minutes
+    n_rows = max(32, min(192, 192 * 300 // max(args.steps, 1)))
     flops_per_row = 4 * cfg.kv_visible[0] * cfg.d
     for i in range(args.warmup):
         rows, heads = wl.sample_pairs(cfg, n_rows, seed=i)
