@@ -188,9 +188,7 @@ class UnitOnDevice:
         if record: ev[0].record()
         ws.kv_cache_write(self.kc, self.vc, s["ks"], s["vs"], 0, cfg.write_offset)
         if record: ev[1].record()
-        ws.seq_to_head(self.q_h, s["q"], 1, 0, 1)
-        ws.seq_to_head(self.kn_h, s["kn"], 1, 0, 1)
-        ws.seq_to_head(self.vn_h, s["vn"], 1, 0, 1)
+        ws.seq_to_head_multi((self.q_h, self.kn_h, self.vn_h), (s["q"], s["kn"], s["vn"]), 1, 0, 1)  # a2 x3, one launch
         if record: ev[2].record()
         ws.block_causal_attn(self.o_h[0], self.q_h[0], self.kc, self.vc, cfg.cache_len, self.kn_h[0], self.vn_h[0],
                              cfg.q_block_end, cfg.kv_visible, cfg.softmax_scale, self.wsp)

@@ -91,6 +91,17 @@ int ws_seq_to_head(void* dst, const void* src, int64_t n_tok, int32_t H, int32_t
 int ws_head_to_seq(void* dst, const void* src, int64_t n_tok, int32_t H, int32_t d, int32_t P,
                    int32_t g0, int32_t G, ws_dtype dt, void* stream);
 
+/* a2 / a4 on several tensors of one shape in ONE launch (at most 4; e.g. Q, K_new and V_new before
+ * attention).  dsts / srcs are HOST arrays of n_tensors device pointers, read during the call only.
+ * Semantics, layouts and errors per tensor exactly as ws_seq_to_head / ws_head_to_seq; in addition no
+ * destination may intersect any source or any other destination (OVERLAP), and n_tensors > 4 is
+ * UNSUPPORTED.  A 10-20 MB relayout is dominated by launch and DRAM round-trip latency:
+ * batching pays it once. */
+int ws_seq_to_head_multi(void* const* dsts, const void* const* srcs, int32_t n_tensors, int64_t n_tok, int32_t H,
+                         int32_t d, int32_t P, int32_t g0, int32_t G, ws_dtype dt, void* stream);
+int ws_head_to_seq_multi(void* const* dsts, const void* const* srcs, int32_t n_tensors, int64_t n_tok, int32_t H,
+                         int32_t d, int32_t P, int32_t g0, int32_t G, ws_dtype dt, void* stream);
+
 /* ------------------------------------------------------------------------------------------------
  * a3. Block-causal unit attention
  *

@@ -20,7 +20,7 @@ _LIB_PATH = os.path.join(_PKG, "libws.so")
 _lib = None
 
 EXPORTS = (
-    "ws_kv_cache_write", "ws_seq_to_head", "ws_head_to_seq", "ws_block_causal_attn_workspace_bytes",
+    "ws_kv_cache_write", "ws_seq_to_head", "ws_head_to_seq", "ws_seq_to_head_multi", "ws_head_to_seq_multi", "ws_block_causal_attn_workspace_bytes",
     "ws_block_causal_attn", "ws_block_causal_attn_seq_layout", "ws_unit_forward_host_staging_bytes", "ws_unit_forward_host", "ws_status_string",
     "ws_version", "ws_last_cuda_error", "ws_kernel_launch_count",
 )
@@ -58,6 +58,9 @@ def load():
     lib.ws_kv_cache_write.restype = ctypes.c_int
     for fn in (lib.ws_seq_to_head, lib.ws_head_to_seq):
         fn.argtypes = [vp, vp, i64, i32, i32, i32, i32, i32, ctypes.c_int, vp]
+        fn.restype = ctypes.c_int
+    for fn in (lib.ws_seq_to_head_multi, lib.ws_head_to_seq_multi):
+        fn.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(vp), i32, i64, i32, i32, i32, i32, i32, ctypes.c_int, vp]
         fn.restype = ctypes.c_int
     lib.ws_block_causal_attn_workspace_bytes.argtypes = [i32, i32, i32, i64, ctypes.c_int]
     lib.ws_block_causal_attn_workspace_bytes.restype = sz
@@ -160,6 +163,35 @@ def head_to_seq(dst, src, P: int, g0: int, G: int, stream=None):
     if P > 0 and H % P == 0 and tuple(src.shape) != (G, n_tok, H // P, d):
         raise ValueError("ws_head_to_seq: src must be [G, n_tok, H/P, d]")
     _ok(load().ws_head_to_seq(_p(dst), _p(src), n_tok, H, d, P, g0, G, _dt(dst), _stream(stream)), "ws_head_to_seq")
+
+
+def _multi(fn_name, toks, heads, P, g0, G, stream, to_head):
+    """toks: token-major [n_tok, H, d] tensors; heads: head-major [G, n_tok, H/P, d] tensors (same shapes throughout)."""
+    if len(toks) != len(heads) or not toks:
+        raise ValueError(f"{fn_name}: need as many sources as destinations (at least one)")
+    _dev(*toks, *heads)
+    n_tok, H, d = toks[0].shape
+    for t, h in zip(toks, heads):
+        if tuple(t.shape) != (n_tok, H, d) or t.dtype != toks[0].dtype or h.dtype != toks[0].dtype:
+            raise ValueError(f"{fn_name}: all tensors must share shape and dtype")
+        if P > 0 and H % P == 0 and tuple(h.shape) != (G, n_tok, H // P, d):
+            raise ValueError(f"{fn_name}: head-major tensors must be [G, n_tok, H/P, d]")
+    n = len(toks)
+    dsts, srcs = (heads, toks) if to_head else (toks, heads)
+    da = (ctypes.c_void_p * n)(*[t.data_ptr() for t in dsts])
+    sa = (ctypes.c_void_p * n)(*[t.data_ptr() for t in srcs])
+    rc = getattr(load(), fn_name)(da, sa, n, n_tok, H, d, P, g0, G, _dt(toks[0]), _stream(stream))
+    _ok(rc, fn_name)
+
+
+def seq_to_head_multi(dsts, srcs, P: int, g0: int, G: int, stream=None):
+    """ws_seq_to_head on up to four same-shaped tensors in one launch (ws.h)."""
+    _multi("ws_seq_to_head_multi", list(srcs), list(dsts), P, g0, G, stream, True)
+
+
+def head_to_seq_multi(dsts, srcs, P: int, g0: int, G: int, stream=None):
+    """ws_head_to_seq on up to four same-shaped tensors in one launch (ws.h)."""
+    _multi("ws_head_to_seq_multi", list(dsts), list(srcs), P, g0, G, stream, False)
 
 
 def block_causal_attn_workspace_bytes(Lq: int, H: int, d: int, kv_total: int, dtype=torch.bfloat16) -> int:

@@ -16,6 +16,12 @@ namespace {
 constexpr int kThreads = 256;
 constexpr int kUnroll = 8;  // 16-byte vectors per thread
 
+constexpr int kMaxTensors = 4;  // tensors moved by one launch (blockIdx.z)
+struct CopyPtrs {
+  const uint4* src[kMaxTensors];
+  uint4* dst[kMaxTensors];
+};
+
 struct CopyPlan {
   uint32_t dv;     // 16-byte vectors per contiguous chunk
   uint32_t per_a;  // B * dv: vectors per outer index a
@@ -31,12 +37,10 @@ __device__ __forceinline__ uint4 ld_stream(const uint4* p) {
 }
 
 // grid = (ceil(per_a / (kThreads*kUnroll)), A, n_tensors)
-__global__ void __launch_bounds__(kThreads) strided_copy16_kernel(const uint4* __restrict__ src0, uint4* __restrict__ dst0,
-                                                                  const uint4* __restrict__ src1, uint4* __restrict__ dst1,
-                                                                  CopyPlan p) {
+__global__ void __launch_bounds__(kThreads) strided_copy16_kernel(const __grid_constant__ CopyPtrs ptrs, const __grid_constant__ CopyPlan p) {
   wsi::pdl_trigger();  // the next kernel may be scheduled now; it blocks in its own pdl_wait() until this grid is done
-  const uint4* __restrict__ src = blockIdx.z == 0 ? src0 : src1;
-  uint4* __restrict__ dst = blockIdx.z == 0 ? dst0 : dst1;
+  const uint4* __restrict__ src = ptrs.src[blockIdx.z];
+  uint4* __restrict__ dst = ptrs.dst[blockIdx.z];
   const int64_t a = blockIdx.y;
   src += a * p.src_a;
   dst += a * p.dst_a;
@@ -63,11 +67,11 @@ __global__ void __launch_bounds__(kThreads) strided_copy16_kernel(const uint4* _
     if (doff[u] >= 0) dst[doff[u]] = v[u];
 }
 
-// Launches the plan, splitting B so that per_a stays below 2^30 vectors.
-int launch_copy(const void* s0, void* d0, const void* s1, void* d1, int n_tensors, int64_t A, int64_t B, int64_t dv,
-                int64_t src_a, int64_t src_b, int64_t dst_a, int64_t dst_b, cudaStream_t stream) {
-  if (A == 0 || B == 0 || dv == 0) return WS_OK;
-  if (A > 65535 || dv > (1 << 20)) return WS_ERR_UNSUPPORTED;
+// Launches the plan for n_tensors (source, destination) pairs of the same shape, splitting B so that per_a stays below 2^30 vectors.
+int launch_copy(const void* const* srcs, void* const* dsts, int n_tensors, int64_t A, int64_t B, int64_t dv, int64_t src_a,
+                int64_t src_b, int64_t dst_a, int64_t dst_b, cudaStream_t stream) {
+  if (A == 0 || B == 0 || dv == 0 || n_tensors == 0) return WS_OK;
+  if (A > 65535 || dv > (1 << 20) || n_tensors > kMaxTensors) return WS_ERR_UNSUPPORTED;
   const int64_t max_b = ((int64_t)1 << 30) / dv;
   int launches = 0;
   for (int64_t b0 = 0; b0 < B; b0 += max_b) {
@@ -76,40 +80,55 @@ int launch_copy(const void* s0, void* d0, const void* s1, void* d1, int n_tensor
     p.dv = (uint32_t)dv;
     p.per_a = (uint32_t)(nb * dv);
     p.src_a = src_a; p.src_b = src_b; p.dst_a = dst_a; p.dst_b = dst_b;
-    const uint4* ps0 = reinterpret_cast<const uint4*>(s0) + b0 * src_b;
-    uint4* pd0 = reinterpret_cast<uint4*>(d0) + b0 * dst_b;
-    const uint4* ps1 = s1 ? reinterpret_cast<const uint4*>(s1) + b0 * src_b : nullptr;
-    uint4* pd1 = d1 ? reinterpret_cast<uint4*>(d1) + b0 * dst_b : nullptr;
+    CopyPtrs ptrs = {};
+    for (int i = 0; i < n_tensors; ++i) {
+      ptrs.src[i] = reinterpret_cast<const uint4*>(srcs[i]) + b0 * src_b;
+      ptrs.dst[i] = reinterpret_cast<uint4*>(dsts[i]) + b0 * dst_b;
+    }
     dim3 grid((unsigned)((p.per_a + kThreads * kUnroll - 1) / (kThreads * kUnroll)), (unsigned)A, (unsigned)n_tensors);
-    const cudaError_t e = wsi::launch_pdl(strided_copy16_kernel, grid, dim3(kThreads), 0, stream, ps0, pd0, ps1, pd1, p);
+    const cudaError_t e = wsi::launch_pdl(strided_copy16_kernel, grid, dim3(kThreads), 0, stream, ptrs, p);
     if (e != cudaSuccess) return wsi::cuda_fail(e);
     ++launches;
   }
   return wsi::after_launch(launches);
 }
 
-int relayout(void* dst, const void* src, int64_t n_tok, int32_t H, int32_t d, int32_t P, int32_t g0, int32_t G, ws_dtype dt,
-             void* stream, bool to_head) {
+int relayout(void* const* dsts, const void* const* srcs, int n_tensors, int64_t n_tok, int32_t H, int32_t d, int32_t P, int32_t g0,
+             int32_t G, ws_dtype dt, void* stream, bool to_head) {
   const int es = wsi::elem_bytes(dt);
   if (es == 0) return WS_ERR_UNSUPPORTED;
-  if (!dst || !src || n_tok < 0 || H <= 0 || d <= 0 || P <= 0 || H % P != 0 || g0 < 0 || G < 0 || g0 + G > P)
+  if (!dsts || !srcs || n_tensors < 0 || n_tok < 0 || H <= 0 || d <= 0 || P <= 0 || H % P != 0 || g0 < 0 || G < 0 || g0 + G > P)
     return WS_ERR_INVALID_ARG;
+  if (n_tensors > kMaxTensors) return WS_ERR_UNSUPPORTED;
   const int32_t Hp = H / P;
   const int64_t chunk_bytes = (int64_t)Hp * d * es;  // contiguous bytes per (g, t)
-  if (!wsi::aligned16(dst) || !wsi::aligned16(src) || ((int64_t)d * es) % 16 != 0) return WS_ERR_ALIGNMENT;
+  if (((int64_t)d * es) % 16 != 0) return WS_ERR_ALIGNMENT;
   const size_t tok_bytes = (size_t)n_tok * H * d * es;          // token-major tensor
   const size_t head_bytes = (size_t)G * n_tok * chunk_bytes;    // head-major tensor
-  if (wsi::ranges_overlap(dst, to_head ? head_bytes : tok_bytes, src, to_head ? tok_bytes : head_bytes)) return WS_ERR_OVERLAP;
+  const size_t dst_bytes = to_head ? head_bytes : tok_bytes, src_bytes = to_head ? tok_bytes : head_bytes;
+  for (int i = 0; i < n_tensors; ++i) {
+    if (!dsts[i] || !srcs[i]) return WS_ERR_INVALID_ARG;
+    if (!wsi::aligned16(dsts[i]) || !wsi::aligned16(srcs[i])) return WS_ERR_ALIGNMENT;
+  }
+  for (int i = 0; i < n_tensors; ++i) {  // no destination may intersect any source or any other destination
+    for (int j = 0; j < n_tensors; ++j) {
+      if (wsi::ranges_overlap(dsts[i], dst_bytes, srcs[j], src_bytes)) return WS_ERR_OVERLAP;
+      if (j != i && wsi::ranges_overlap(dsts[i], dst_bytes, dsts[j], dst_bytes)) return WS_ERR_OVERLAP;
+    }
+  }
   const int64_t dv = chunk_bytes / 16;
   const int64_t tok_a = (int64_t)Hp * d * es / 16;   // token-major: group g -> + g * Hp heads
   const int64_t tok_b = (int64_t)H * d * es / 16;    // token t
   const int64_t head_a = n_tok * dv;                 // head-major: group g
   const int64_t head_b = dv;                         // token t
-  const char* tok_base_c = reinterpret_cast<const char*>(to_head ? src : dst) + (int64_t)g0 * chunk_bytes;
-  if (to_head)
-    return launch_copy(tok_base_c, dst, nullptr, nullptr, 1, G, n_tok, dv, tok_a, tok_b, head_a, head_b, (cudaStream_t)stream);
-  return launch_copy(src, const_cast<char*>(tok_base_c), nullptr, nullptr, 1, G, n_tok, dv, head_a, head_b, tok_a, tok_b,
-                     (cudaStream_t)stream);
+  const void* s2[kMaxTensors];
+  void* d2[kMaxTensors];
+  for (int i = 0; i < n_tensors; ++i) {  // the token-major side starts at the first selected head group
+    s2[i] = to_head ? static_cast<const void*>(reinterpret_cast<const char*>(srcs[i]) + (int64_t)g0 * chunk_bytes) : srcs[i];
+    d2[i] = to_head ? dsts[i] : static_cast<void*>(reinterpret_cast<char*>(dsts[i]) + (int64_t)g0 * chunk_bytes);
+  }
+  if (to_head) return launch_copy(s2, d2, n_tensors, G, n_tok, dv, tok_a, tok_b, head_a, head_b, (cudaStream_t)stream);
+  return launch_copy(s2, d2, n_tensors, G, n_tok, dv, head_a, head_b, tok_a, tok_b, (cudaStream_t)stream);
 }
 
 }  // namespace
@@ -142,15 +161,29 @@ extern "C" __attribute__((visibility("default"))) int ws_kv_cache_write(void* k_
   const char* vs = reinterpret_cast<const char*>(v_src) + (int64_t)head_begin * row_bytes;
   char* kd = reinterpret_cast<char*>(k_cache) + row_offset * row_bytes;
   char* vd = reinterpret_cast<char*>(v_cache) + row_offset * row_bytes;
-  return launch_copy(ks, kd, vs, vd, 2, H, n_rows, dv, dv, (int64_t)H_src * dv, capacity * dv, dv, (cudaStream_t)stream);
+  const void* srcs2[2] = {ks, vs};
+  void* dsts2[2] = {kd, vd};
+  return launch_copy(srcs2, dsts2, 2, H, n_rows, dv, dv, (int64_t)H_src * dv, capacity * dv, dv, (cudaStream_t)stream);
 }
 
 extern "C" __attribute__((visibility("default"))) int ws_seq_to_head(void* dst, const void* src, int64_t n_tok, int32_t H, int32_t d, int32_t P, int32_t g0, int32_t G,
                               ws_dtype dt, void* stream) {
-  return relayout(dst, src, n_tok, H, d, P, g0, G, dt, stream, true);
+  return relayout(&dst, &src, 1, n_tok, H, d, P, g0, G, dt, stream, true);
 }
 
 extern "C" __attribute__((visibility("default"))) int ws_head_to_seq(void* dst, const void* src, int64_t n_tok, int32_t H, int32_t d, int32_t P, int32_t g0, int32_t G,
                               ws_dtype dt, void* stream) {
-  return relayout(dst, src, n_tok, H, d, P, g0, G, dt, stream, false);
+  return relayout(&dst, &src, 1, n_tok, H, d, P, g0, G, dt, stream, false);
+}
+
+// Several tensors of one shape in ONE launch (Q, K_new and V_new before attention): the launch and DRAM round-trip
+// latency that dominates a 10-20 MB relayout is paid once.
+extern "C" __attribute__((visibility("default"))) int ws_seq_to_head_multi(void* const* dsts, const void* const* srcs, int32_t n_tensors, int64_t n_tok,
+                                    int32_t H, int32_t d, int32_t P, int32_t g0, int32_t G, ws_dtype dt, void* stream) {
+  return relayout(dsts, srcs, n_tensors, n_tok, H, d, P, g0, G, dt, stream, true);
+}
+
+extern "C" __attribute__((visibility("default"))) int ws_head_to_seq_multi(void* const* dsts, const void* const* srcs, int32_t n_tensors, int64_t n_tok,
+                                    int32_t H, int32_t d, int32_t P, int32_t g0, int32_t G, ws_dtype dt, void* stream) {
+  return relayout(dsts, srcs, n_tensors, n_tok, H, d, P, g0, G, dt, stream, false);
 }

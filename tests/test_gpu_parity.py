@@ -119,6 +119,43 @@ def test_relayouts_bit_exact_and_round_trip(n_tok, H, d, P, g0, G, dtype):
     assert np.array_equal(got[:, sel], src[:, sel]) and np.all(got[:, ~sel] == 0x7EEE)
 
 
+def test_multi_tensor_relayouts_equal_single_calls():
+    """ws_seq_to_head_multi / ws_head_to_seq_multi: three tensors in one launch == three single calls == oracle."""
+    n_tok, H, d, P, g0, G = 970, 40, 128, 4, 1, 2
+    rng = np.random.default_rng(21)
+    srcs_np = [wl.bf16_round(rng.standard_normal((n_tok, H, d), dtype=np.float32)) for _ in range(3)]
+    srcs = [to_dev(a, "bf16") for a in srcs_np]
+    one = [torch.full((G, n_tok, H // P, d), 7.0, dtype=torch.bfloat16, device="cuda") for _ in range(3)]
+    many = [torch.full_like(o, 9.0) for o in one]
+    for o, a in zip(one, srcs):
+        ws.seq_to_head(o, a, P, g0, G)
+    ws.seq_to_head_multi(many, srcs, P, g0, G)
+    torch.cuda.synchronize()
+    for o, m, a in zip(one, many, srcs_np):
+        assert np.array_equal(raw_bytes(o), raw_bytes(m))
+        ref = np.empty((G, n_tok, H // P, d), np.float32)
+        wsref.seq_to_head(ref, a, P, g0, G)
+        assert np.array_equal(to_host(m), ref)
+    back_one = [torch.full((n_tok, H, d), 3.0, dtype=torch.bfloat16, device="cuda") for _ in range(3)]
+    back_many = [torch.full_like(b, 3.0) for b in back_one]
+    for b, m in zip(back_one, many):
+        ws.head_to_seq(b, m, P, g0, G)
+    ws.head_to_seq_multi(back_many, many, P, g0, G)
+    torch.cuda.synchronize()
+    for b, m in zip(back_one, back_many):
+        assert np.array_equal(raw_bytes(b), raw_bytes(m))
+    # errors: too many tensors, overlapping destinations -- nothing is written
+    with pytest.raises(ws.WsError) as e:
+        ws.seq_to_head_multi(many + many[:2], srcs + srcs[:2], P, g0, G)
+    assert e.value.status == -2
+    before = raw_bytes(many[0]).copy()
+    with pytest.raises(ws.WsError) as e:
+        ws.seq_to_head_multi([many[0], many[0]], srcs[:2], P, g0, G)
+    assert e.value.status == -5
+    torch.cuda.synchronize()
+    assert np.array_equal(raw_bytes(many[0]), before)
+
+
 # ================================================================================================
 # a3: attention -- BASELINE.json configs (config 1 whole; 2-5 reduced copies whole, full size sampled)
 # ================================================================================================
