@@ -482,7 +482,7 @@ def run_ours(args):
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
         "data": "synthetic", "impl": "ours",
         "config": {"workload": "cfg3: 640x368 unit, 970 queries (920 video + 50 audio) x 40 heads x d128, cache 16384 + own 970 keys, "
-                               "1024-row K/V slice written first; step = cache write + 3x seq->head + attention + head->seq (P=1)",
+                               "1024-row K/V slice written first; step = cache write + seq->head of Q, K_new, V_new (one launch) + attention + head->seq (P=1)",
                    "l2_policy": "inputs larger than L2 (335 MB K/V cache per step vs 126 MB L2) and two rotating input sets",
                    "seed": cfg.seed, "flops_per_step": flops, "replicas": world},
         "e2e": {"value": flops * e2e_units / e2e_ms / 1e9, "unit": "TFLOP/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
