@@ -206,6 +206,16 @@ int ws_unit_forward_host(void* out_host, const void* q_host, const void* k_new_h
                          int64_t cache_len_after, int32_t H, int32_t d, float softmax_scale, void* staging,
                          size_t staging_bytes, void* stream);
 
+/* Host-only diagnostic (touches no device): the work schedule ws_block_causal_attn would use for this problem on
+ * a device with n_sms SMs ("Schedule").  Work item i = head * n_pairs + pair, n_pairs =
+ * ceil(Lq / 256); pair p has pair_tiles[p] KV-tile iterations.  CTA c < *grid runs the whole items w * grid + c
+ * for w < *n_waves, then the flattened iterations [pool_begin[c], pool_begin[c + 1]) of the remaining items
+ * (coordinate of item i, tile j: (i / n_pairs) * sum(pair_tiles) + sum(pair_tiles[0 .. i % n_pairs)) + j).
+ *   pair_tiles : host, >= ceil(Lq / 256) entries (written);  pool_begin : host, >= n_sms + 1 entries (written)
+ * Errors: INVALID_ARG, OUT_OF_RANGE, UNSUPPORTED as for the mask of ws_block_causal_attn. */
+int ws_attn_schedule(int32_t Lq, int32_t H, int64_t cache_len, int32_t Ln, const ws_block_mask* mask, int32_t n_sms,
+                     int32_t* grid, int32_t* n_waves, int32_t* pair_tiles, int64_t* pool_begin);
+
 /* ---- utilities ---- */
 const char* ws_status_string(int status); /* static string, never NULL */
 int ws_version(void);                     /* WS_VERSION of the loaded library */

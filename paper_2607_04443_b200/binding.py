@@ -22,7 +22,7 @@ _lib = None
 EXPORTS = (
     "ws_kv_cache_write", "ws_seq_to_head", "ws_head_to_seq", "ws_seq_to_head_multi", "ws_head_to_seq_multi", "ws_block_causal_attn_workspace_bytes",
     "ws_block_causal_attn", "ws_block_causal_attn_seq_layout", "ws_unit_forward_host_staging_bytes", "ws_unit_forward_host", "ws_status_string",
-    "ws_version", "ws_last_cuda_error", "ws_kernel_launch_count",
+    "ws_version", "ws_last_cuda_error", "ws_kernel_launch_count", "ws_attn_schedule",
 )
 
 
@@ -75,6 +75,9 @@ def load():
     lib.ws_unit_forward_host.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp, i64, vp, vp, i32, i64, i64, i32, i32, f32,
                                          vp, sz, vp]
     lib.ws_unit_forward_host.restype = ctypes.c_int
+    lib.ws_attn_schedule.argtypes = [i32, i32, i64, i32, ctypes.POINTER(_BlockMask), i32, ctypes.POINTER(i32), ctypes.POINTER(i32),
+                                     ctypes.POINTER(i32), ctypes.POINTER(i64)]
+    lib.ws_attn_schedule.restype = ctypes.c_int
     lib.ws_status_string.argtypes = [ctypes.c_int]
     lib.ws_status_string.restype = ctypes.c_char_p
     for fn in (lib.ws_version, lib.ws_last_cuda_error, lib.ws_kernel_launch_count):
@@ -260,6 +263,22 @@ def block_causal_attn_seq_layout(out_seq, q_seq, k_cache, v_cache, cache_len: in
                                                 ctypes.byref(mask), float(softmax_scale), _p(workspace),
                                                 workspace.numel() * workspace.element_size(), _dt(q_seq), _stream(stream))
     _ok(rc, "ws_block_causal_attn_seq_layout")
+
+
+def attn_schedule(Lq: int, H: int, cache_len: int, Ln: int, q_block_end: Sequence[int], kv_visible: Sequence[int], n_sms: int):
+    """Host-only: the attention work schedule for a device with n_sms SMs (ws.h ws_attn_schedule).
+    Returns dict(grid, n_waves, pair_tiles [n_pairs], pool_begin [grid + 1])."""
+    n = len(q_block_end)
+    qe = (ctypes.c_int32 * n)(*[int(x) for x in q_block_end])
+    kv = (ctypes.c_int32 * n)(*[int(x) for x in kv_visible])
+    mask = _BlockMask(n, qe, kv)
+    n_pairs = (Lq + 255) // 256
+    grid, waves = ctypes.c_int32(0), ctypes.c_int32(0)
+    tiles = (ctypes.c_int32 * max(n_pairs, 1))()
+    pool = (ctypes.c_int64 * (n_sms + 1))()
+    rc = load().ws_attn_schedule(Lq, H, int(cache_len), Ln, ctypes.byref(mask), n_sms, ctypes.byref(grid), ctypes.byref(waves), tiles, pool)
+    _ok(rc, "ws_attn_schedule")
+    return dict(grid=grid.value, n_waves=waves.value, pair_tiles=list(tiles)[:n_pairs], pool_begin=list(pool)[:grid.value + 1])
 
 
 def unit_forward_host_staging_bytes(Lq, Ln, H, d, n_slice_rows, kv_total, n_steps) -> int:

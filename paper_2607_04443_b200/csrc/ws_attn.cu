@@ -800,6 +800,107 @@ extern "C" __attribute__((visibility("default"))) size_t ws_block_causal_attn_wo
 }
 
 namespace {
+// KV-tile iterations of every Q-tile pair: a pair visits the KV tiles its last row can see.  Fills
+// prm.pair_prefix / n_cache_tiles (needs prm.n_pairs) and returns the iterations per head.
+int64_t build_pair_prefix(Params& prm, const ws_block_mask* mask, int32_t Lq, int64_t cache_len) {
+  prm.n_cache_tiles = (int)((cache_len + kBlockN - 1) / kBlockN);
+  int64_t Tp = 0;
+  prm.pair_prefix[0] = 0;
+  for (int pr = 0; pr < prm.n_pairs; ++pr) {
+    const int last_row = ((pr + 1) * kPairM < Lq ? (pr + 1) * kPairM : Lq) - 1;
+    int b = 0;
+    while (last_row >= mask->q_block_end[b]) ++b;
+    const int64_t nvis = mask->kv_visible[b];
+    if (nvis > 0)
+      Tp += nvis <= cache_len ? (nvis + kBlockN - 1) / kBlockN : prm.n_cache_tiles + (nvis - cache_len + kBlockN - 1) / kBlockN;
+    prm.pair_prefix[pr + 1] = (int32_t)Tp;
+  }
+  return Tp;
+}
+
+// The two-phase schedule (see Params) for a device with `sms` SMs: fills prm.grid, n_waves, pool_begin.
+void build_schedule(Params& prm, int64_t Tp, int sms) {
+  const int n_pairs = prm.n_pairs, H = prm.H;
+  const int64_t T = Tp * H, n_items = (int64_t)H * n_pairs;
+  int64_t G = T > 0 ? T : n_items;
+  if (G > sms) G = sms;
+  if (G > kMaxCtas) G = kMaxCtas;
+  prm.grid = (int32_t)G;
+  auto item_len = [&](int64_t i) { const int pr = (int)(i % n_pairs); return (int64_t)(prm.pair_prefix[pr + 1] - prm.pair_prefix[pr]); };
+  auto item_flat = [&](int64_t i) { return (i / n_pairs) * Tp + prm.pair_prefix[i % n_pairs]; };
+  // candidate B: W whole-item waves, the remaining items water-filled over the CTAs
+  const int64_t W = n_items / G;
+  int64_t p1[kMaxCtas], quota[kMaxCtas];
+  int64_t pool = T, p1_max = 0;
+  for (int64_t c = 0; c < G; ++c) {
+    p1[c] = 0;
+    for (int64_t w = 0; w < W; ++w) p1[c] += item_len(w * G + c);
+    pool -= p1[c];
+    if (p1[c] > p1_max) p1_max = p1[c];
+  }
+  // smallest level with sum_c max(0, level - p1[c]) >= pool
+  int64_t lo = 0, hi = p1_max + pool;
+  while (lo < hi) {
+    const int64_t mid = (lo + hi) / 2;
+    int64_t cap = 0;
+    for (int64_t c = 0; c < G; ++c) cap += mid > p1[c] ? mid - p1[c] : 0;
+    if (cap >= pool) hi = mid; else lo = mid + 1;
+  }
+  int64_t excess = -pool;
+  for (int64_t c = 0; c < G; ++c) { quota[c] = lo > p1[c] ? lo - p1[c] : 0; excess += quota[c]; }
+  for (int64_t c = G - 1; c >= 0 && excess > 0; --c)
+    if (quota[c] > 0) { --quota[c]; --excess; }
+  const int64_t makespan_b = lo > p1_max ? lo : p1_max, makespan_a = (T + G - 1) / G;
+  // B trades a slightly longer critical path for far fewer split items and L2 reuse of K/V across the pairs of a head
+  const bool use_b = W > 0 && makespan_b * 100 <= makespan_a * 103;
+  if (use_b) {
+    prm.n_waves = (int32_t)W;
+    int64_t t = item_flat(W * G);
+    for (int64_t c = 0; c < G; ++c) { prm.pool_begin[c] = t; t += quota[c]; }
+    prm.pool_begin[G] = t;  // == T
+  } else {
+    prm.n_waves = 0;
+    for (int64_t c = 0; c <= G; ++c) prm.pool_begin[c] = (c * T) / G;
+  }
+}
+
+// The mask rules shared by the attention entry points and the schedule diagnostic.
+int check_mask(const ws_block_mask* mask, int32_t Lq, int64_t cache_len, int32_t Ln) {
+  if (!mask || mask->n_blocks <= 0 || !mask->q_block_end || !mask->kv_visible) return WS_ERR_INVALID_ARG;
+  if (mask->n_blocks > WS_MAX_MASK_BLOCKS) return WS_ERR_UNSUPPORTED;
+  int32_t prev_end = 0, prev_vis = 0;
+  for (int b = 0; b < mask->n_blocks; ++b) {
+    if (mask->q_block_end[b] <= prev_end || mask->kv_visible[b] < prev_vis) return WS_ERR_INVALID_ARG;
+    if ((int64_t)mask->kv_visible[b] > cache_len + Ln) return WS_ERR_OUT_OF_RANGE;
+    prev_end = mask->q_block_end[b];
+    prev_vis = mask->kv_visible[b];
+  }
+  return prev_end == Lq ? WS_OK : WS_ERR_INVALID_ARG;
+}
+}  // namespace
+
+// Host-only diagnostic: the schedule ws_block_causal_attn uses for this problem on a device with n_sms SMs.
+extern "C" __attribute__((visibility("default"))) int ws_attn_schedule(int32_t Lq, int32_t H, int64_t cache_len, int32_t Ln, const ws_block_mask* mask,
+                                int32_t n_sms, int32_t* grid, int32_t* n_waves, int32_t* pair_tiles, int64_t* pool_begin) {
+  if (Lq <= 0 || H <= 0 || cache_len < 0 || Ln < 0 || n_sms <= 0 || !grid || !n_waves || !pair_tiles || !pool_begin)
+    return WS_ERR_INVALID_ARG;
+  if (const int rc = check_mask(mask, Lq, cache_len, Ln)) return rc;
+  if (cache_len + Ln > 0x7fffffffLL / kMaxPairs - kBlockN) return WS_ERR_UNSUPPORTED;
+  Params* prm = new Params();
+  prm->Lq = Lq; prm->H = H; prm->Ln = Ln; prm->cache_len = cache_len;
+  prm->n_pairs = (Lq + kPairM - 1) / kPairM;
+  if (prm->n_pairs > kMaxPairs) { delete prm; return WS_ERR_UNSUPPORTED; }
+  const int64_t Tp = build_pair_prefix(*prm, mask, Lq, cache_len);
+  build_schedule(*prm, Tp, n_sms);
+  *grid = prm->grid;
+  *n_waves = prm->n_waves;
+  for (int pr = 0; pr < prm->n_pairs; ++pr) pair_tiles[pr] = prm->pair_prefix[pr + 1] - prm->pair_prefix[pr];
+  for (int c = 0; c <= prm->grid; ++c) pool_begin[c] = prm->pool_begin[c];
+  delete prm;
+  return WS_OK;
+}
+
+namespace {
 // Shared implementation.  q / k_new / v_new / out are token-major with `tok_heads` heads per token in memory, of which
 // the H heads starting at the given base pointers take part (tok_heads == H for the plain [L, H, d] call).
 int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const void* v_cache, int64_t capacity,
@@ -891,64 +992,11 @@ int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const v
     prm.q_block_end[b] = mask->q_block_end[b];
     prm.kv_visible[b] = mask->kv_visible[b];
   }
-  // total KV-tile iterations (host copy of the device schedule)
-  // the schedule: a Q-tile pair visits the KV tiles its last row can see
-  int64_t Tp = 0;
-  prm.pair_prefix[0] = 0;
-  for (int pr = 0; pr < n_pairs; ++pr) {
-    const int last_row = ((pr + 1) * kPairM < Lq ? (pr + 1) * kPairM : Lq) - 1;
-    int b = 0;
-    while (last_row >= mask->q_block_end[b]) ++b;
-    const int64_t nvis = mask->kv_visible[b];
-    if (nvis > 0)
-      Tp += nvis <= cache_len ? (nvis + kBlockN - 1) / kBlockN : prm.n_cache_tiles + (nvis - cache_len + kBlockN - 1) / kBlockN;
-    prm.pair_prefix[pr + 1] = (int32_t)Tp;
-  }
-  // ---- two-phase schedule (see Params) ----
+  const int64_t Tp = build_pair_prefix(prm, mask, Lq, cache_len);
   {
     const int sms = sm_count();
     if (sms <= 0) return wsi::cuda_fail(cudaErrorNoDevice);
-    const int64_t T = Tp * H, n_items = (int64_t)H * n_pairs;
-    int64_t G = T > 0 ? T : n_items;
-    if (G > sms) G = sms;
-    if (G > kMaxCtas) G = kMaxCtas;
-    prm.grid = (int32_t)G;
-    auto item_len = [&](int64_t i) { const int pr = (int)(i % n_pairs); return (int64_t)(prm.pair_prefix[pr + 1] - prm.pair_prefix[pr]); };
-    auto item_flat = [&](int64_t i) { return (i / n_pairs) * Tp + prm.pair_prefix[i % n_pairs]; };
-    // candidate B: W whole-item waves, the remaining items water-filled over the CTAs
-    const int64_t W = n_items / G;
-    int64_t p1[kMaxCtas], quota[kMaxCtas];
-    int64_t pool = T, p1_max = 0;
-    for (int64_t c = 0; c < G; ++c) {
-      p1[c] = 0;
-      for (int64_t w = 0; w < W; ++w) p1[c] += item_len(w * G + c);
-      pool -= p1[c];
-      if (p1[c] > p1_max) p1_max = p1[c];
-    }
-    // smallest level with sum_c max(0, level - p1[c]) >= pool
-    int64_t lo = 0, hi = p1_max + pool;
-    while (lo < hi) {
-      const int64_t mid = (lo + hi) / 2;
-      int64_t cap = 0;
-      for (int64_t c = 0; c < G; ++c) cap += mid > p1[c] ? mid - p1[c] : 0;
-      if (cap >= pool) hi = mid; else lo = mid + 1;
-    }
-    int64_t excess = -pool;
-    for (int64_t c = 0; c < G; ++c) { quota[c] = lo > p1[c] ? lo - p1[c] : 0; excess += quota[c]; }
-    for (int64_t c = G - 1; c >= 0 && excess > 0; --c)
-      if (quota[c] > 0) { --quota[c]; --excess; }
-    const int64_t makespan_b = lo > p1_max ? lo : p1_max, makespan_a = (T + G - 1) / G;
-    // B trades a slightly longer critical path for far fewer split items and L2 reuse of K/V across the pairs of a head
-    const bool use_b = W > 0 && makespan_b * 100 <= makespan_a * 103;
-    if (use_b) {
-      prm.n_waves = (int32_t)W;
-      int64_t t = item_flat(W * G);
-      for (int64_t c = 0; c < G; ++c) { prm.pool_begin[c] = t; t += quota[c]; }
-      prm.pool_begin[G] = t;  // == T
-    } else {
-      prm.n_waves = 0;
-      for (int64_t c = 0; c <= G; ++c) prm.pool_begin[c] = (c * T) / G;
-    }
+    build_schedule(prm, Tp, sms);
   }
   if (launches) wsi::count_launch(launches);
   const bool f32 = dt == WS_DTYPE_F32;
