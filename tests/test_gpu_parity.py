@@ -482,3 +482,54 @@ def test_unit_forward_host_matches_oracle():
         q, rkc, rvc, kn, vn = oracle_inputs(cfg, x, s)
         ref, _ = wsref.block_causal_attn(q, rkc, rvc, cfg.cache_len, kn, vn, cfg.q_block_end, cfg.kv_visible, cfg.softmax_scale)
         check_attn(got[s], ref, what=f"host entry step {s}")
+
+
+def test_unit_forward_host_pipelined_over_head_groups():
+    """H = 8: ws_unit_forward_host runs as four head groups (2-D copies on the internal streams, cache write and
+    fused token-major attention per group); cache and every step's output against the oracle."""
+    rng = np.random.default_rng(31)
+    H, d, Lq, Tc0, n_w, cap, steps = 8, 64, 300, 500, 100, 700, 2
+    r = lambda *s: wl.bf16_round(rng.standard_normal(s, dtype=np.float32))
+    k_cache, v_cache = np.zeros((H, cap, d), np.float32), np.zeros((H, cap, d), np.float32)
+    k_cache[:, :Tc0], v_cache[:, :Tc0] = r(H, Tc0, d), r(H, Tc0, d)
+    k_slice, v_slice = r(n_w, H, d), r(n_w, H, d)
+    q, kn, vn = r(steps, Lq, H, d), r(steps, Lq, H, d), r(steps, Lq, H, d)
+    Tc, scale = Tc0 + n_w, 1.0 / math.sqrt(d)
+    host = lambda a: torch.from_numpy(wl.bf16_bits(a).view(np.int16)).view(torch.bfloat16).pin_memory()
+    kc, vc = to_dev(k_cache, "bf16"), to_dev(v_cache, "bf16")
+    outh = torch.zeros((steps, Lq, H, d), dtype=torch.bfloat16).pin_memory()
+    staging = torch.empty(ws.unit_forward_host_staging_bytes(Lq, Lq, H, d, n_w, Tc + Lq, steps), dtype=torch.uint8, device="cuda")
+    for _ in range(2):  # twice: the helper streams and events are reused across calls
+        ws.unit_forward_host(outh, host(q), host(kn), host(vn), kc, vc, host(k_slice), host(v_slice), Tc0, Tc, scale, staging)
+        torch.cuda.synchronize()
+    rk, rv = k_cache.copy(), v_cache.copy()
+    wsref.kv_cache_write(rk, rv, k_slice, v_slice, 0, Tc0)
+    assert np.array_equal(to_host(kc), rk) and np.array_equal(to_host(vc), rv)
+    got = wl.bf16_from_bits(outh.view(torch.int16).numpy().view(np.uint16))
+    for s in range(steps):
+        ref, _ = wsref.block_causal_attn(q[s], rk, rv, Tc, kn[s], vn[s], [Lq], [Tc + Lq], scale)
+        check_attn(got[s], ref, what=f"pipelined host entry step {s}")
+
+
+def test_fused_relayout_attention_in_fp32():
+    """Config-1 arithmetic (FP32 in, rounded to BF16 on the device, FP32 out) through the token-major call:
+    the staging cast gathers the rank's heads token by token."""
+    rng = np.random.default_rng(32)
+    H_total, Hp, d, Lq, Tc, g0 = 4, 2, 64, 64, 128, 1
+    r = lambda *s: rng.standard_normal(s, dtype=np.float32)
+    q, kn, vn = r(Lq, H_total, d), r(Lq, H_total, d), r(Lq, H_total, d)
+    k_cache, v_cache = r(Hp, Tc, d), r(Hp, Tc, d)
+    qe, kv, scale = [32, 64], [Tc + 32, Tc + 64], 1.0 / math.sqrt(d)
+    tq, tkn, tvn = to_dev(q, "f32"), to_dev(kn, "f32"), to_dev(vn, "f32")
+    tkc, tvc = to_dev(k_cache, "f32"), to_dev(v_cache, "f32")
+    wsp = workspace_for(Lq, Hp, d, Tc + Lq, torch.float32)
+    out = torch.full_like(tq, 5.0)
+    lse = torch.empty((Hp, Lq), dtype=torch.float32, device="cuda")
+    ws.block_causal_attn_seq_layout(out, tq, tkc, tvc, Tc, tkn, tvn, g0 * Hp, qe, kv, scale, wsp, lse=lse)
+    torch.cuda.synchronize()
+    got = to_host(out)
+    sel = slice(g0 * Hp, (g0 + 1) * Hp)
+    ref, ref_lse = wsref.block_causal_attn(np.ascontiguousarray(q[:, sel]), k_cache, v_cache, Tc, np.ascontiguousarray(kn[:, sel]),
+                                           np.ascontiguousarray(vn[:, sel]), qe, kv, scale)
+    check_attn(got[:, sel], ref, lse.cpu().numpy(), ref_lse, what="fused fp32")
+    assert np.all(got[:, :g0 * Hp] == 5.0), "heads of other ranks must not be touched"
