@@ -435,7 +435,7 @@ def cpu_oracle_sample(cfg, x, target_seconds: float = 12.0):
     wsref.block_causal_attn_rows(*args, rows, heads)
     dt = time.perf_counter() - t
     return {"value": flops_per_row * len(rows) / dt / 1e12, "unit": "TFLOP/s", "cores": wsref.num_threads(), "kind": "oracle",
-            "sample": f"{len(rows)} of {cfg.Lq * cfg.H} (row, head) outputs of {cfg.name}, FP64, {dt:.1f} s",
+            "sample": f"{len(rows)} (row, head) outputs sampled from the {cfg.Lq * cfg.H} of {cfg.name}, FP64, {dt:.1f} s",
             "seconds": dt}, args
 
 

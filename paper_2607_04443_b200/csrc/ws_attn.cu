@@ -766,9 +766,6 @@ int launch_attention(const Params& prm, cudaStream_t stream) {
     attr_err = cudaFuncSetAttribute(attn_fwd_kernel<D, OUT_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes);
   });
   if (attr_err != cudaSuccess) return wsi::cuda_fail(attr_err);
-  const int sms = sm_count();
-  if (sms <= 0) return wsi::cuda_fail(cudaErrorNoDevice);
-  (void)sms;
   int launches = 0;
   if (prm.grid > 0) {
     const cudaError_t e = wsi::launch_pdl(attn_fwd_kernel<D, OUT_F32>, dim3(prm.grid), dim3(kThreads), C::kSmemBytes, stream, prm);
@@ -916,19 +913,8 @@ int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const v
   if ((Ln > 0) != (k_new != nullptr) || (Ln > 0) != (v_new != nullptr)) return WS_ERR_INVALID_ARG;
   if (cache_len > capacity) return WS_ERR_OUT_OF_RANGE;
   if (cache_len > 0 && (!k_cache || !v_cache)) return WS_ERR_INVALID_ARG;
-  if (mask->n_blocks <= 0 || !mask->q_block_end || !mask->kv_visible) return WS_ERR_INVALID_ARG;
-  if (mask->n_blocks > WS_MAX_MASK_BLOCKS) return WS_ERR_UNSUPPORTED;
   if (cache_len + Ln > 0x7fffffffLL / kMaxPairs - kBlockN) return WS_ERR_UNSUPPORTED;  // pair_prefix is int32
-  {
-    int32_t prev_end = 0, prev_vis = 0;
-    for (int b = 0; b < mask->n_blocks; ++b) {
-      if (mask->q_block_end[b] <= prev_end || mask->kv_visible[b] < prev_vis) return WS_ERR_INVALID_ARG;
-      if ((int64_t)mask->kv_visible[b] > cache_len + Ln) return WS_ERR_OUT_OF_RANGE;
-      prev_end = mask->q_block_end[b];
-      prev_vis = mask->kv_visible[b];
-    }
-    if (prev_end != Lq) return WS_ERR_INVALID_ARG;
-  }
+  if (const int rc = check_mask(mask, Lq, cache_len, Ln)) return rc;
   const int n_pairs = (Lq + kPairM - 1) / kPairM;
   if (n_pairs > kMaxPairs) return WS_ERR_UNSUPPORTED;
   if (!wsi::aligned16(out) || !wsi::aligned16(q) || !wsi::aligned16(k_cache) || !wsi::aligned16(v_cache) ||
