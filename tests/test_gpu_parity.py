@@ -316,6 +316,8 @@ SHAPES = [
     (10, 40, 128, [1100], [400], 300, 100),                # 200 equal items: one wave + a 52-item pool
     (11, 160, 64, [256, 300], [0, 450], 200, 250),         # 480 items, three waves; every pair 0 sees no key at all
     (12, 30, 128, [256] * 6, [300, 600, 900, 1200, 1500, 1800], 1500, 300),  # 180 items of very unequal length
+    (13, 2, 128, [100, 100], [128, 256], 256, 50),         # own K/V rows passed but never visible; limits on tile multiples
+    (14, 3, 64, [1], [1], 1, 0),                           # one query, one key
 ]
 
 
