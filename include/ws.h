@@ -11,7 +11,10 @@
  *   ws_block_causal_attn   the unit's latent query tokens attend, "coordinated by block-causal
  *                           attention", to the cached K/V conditioning plus the unit's own K/V
  *                                                                   PAPER.md:25, :73, :79
+ *   ws_block_causal_attn_seq_layout   the two relayouts folded into the attention call (strided TMA)
+ *   ws_seq_to_head_multi / ws_head_to_seq_multi   several same-shaped tensors in one launch
  *   ws_unit_forward_host   the same path for one unit fed from HOST buffers (end-to-end entry)
+ *   ws_attn_schedule       host-only diagnostic: the attention work schedule for a given SM count
  *
  * Conventions (all functions)
  *   - Return value: WS_OK (0) or a negative ws_status.  On any error NOTHING is launched and no
@@ -22,6 +25,8 @@
  *     16 (WS_ERR_ALIGNMENT otherwise).
  *   - No allocation, no synchronisation, no host read of device data: every call is legal
  *     inside CUDA stream capture.  `stream` is a cudaStream_t passed as void* (NULL = default).
+ *     Kernels are launched with programmatic stream serialisation (their set-up overlaps the tail
+ *     of the previous kernel; they wait for it before touching global memory).
  *   - Batch is 1 (fold a batch into heads).  Layouts are dense row-major with the last index
  *     fastest: token-major [L, H, d] for Q / K_new / V_new / O / slices, head-major
  *     [H, capacity, d] for the cache (private to the rank; reading R5).
