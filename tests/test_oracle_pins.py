@@ -466,3 +466,35 @@ def test_config_work_figures_match_survey():
     assert abs(wl.CONFIGS["cfg4"].attn_flops() / 1e9 - 352.04) < 0.01
     assert abs(wl.CONFIGS["cfg5"].attn_flops() / 1e9 - 1321.18) < 0.01
     assert wl.CONFIGS["cfg3"].cache_len == 16384 and wl.CONFIGS["cfg5"].cache_len == 65536
+
+
+def test_parity_metrics_against_hand_values():
+    """wsref.parity_metrics is what every attention parity assert goes through (north_star: max-abs error and
+    relative Frobenius error of the GPU result against the oracle).  Hand values, chosen so that dividing by
+    the wrong norm, dropping the abs, or squaring once too often/too seldom fails."""
+    # got = (3, 4, 0), ref = (0, 0, 5): diff = (3, 4, -5); max|diff| = 5; |diff|_F = sqrt(50); |ref|_F = 5
+    ma, rf = wsref.parity_metrics([3.0, 4.0, 0.0], [0.0, 0.0, 5.0])
+    assert ma == 5.0 and abs(rf - math.sqrt(2.0)) < 1e-15
+    # |got|_F = 5 too, so swap the magnitudes: got = (6, 8), ref = (3, 4): diff = (3, 4); rel = 5 / 5 = 1 (not 5 / 10)
+    ma, rf = wsref.parity_metrics([6.0, 8.0], [3.0, 4.0])
+    assert ma == 4.0 and abs(rf - 1.0) < 1e-15
+    # the largest deviation is negative: abs must be taken before the max
+    ma, rf = wsref.parity_metrics([[1.0, -7.0]], [[1.5, 1.0]])
+    assert ma == 8.0 and abs(rf - math.sqrt(0.25 + 64.0) / math.sqrt(3.25)) < 1e-15
+    # a sign flip of the whole tensor is a relative error of exactly 2
+    x = np.array([[1.0, -2.0], [2.0, 4.0]])
+    ma, rf = wsref.parity_metrics(-x, x)
+    assert ma == 8.0 and abs(rf - 2.0) < 1e-15
+    # identical tensors; an all-zero reference falls back to the absolute norm; empty tensors
+    assert wsref.parity_metrics(x, x) == (0.0, 0.0)
+    ma, rf = wsref.parity_metrics([3.0, 4.0], [0.0, 0.0])
+    assert ma == 4.0 and rf == 5.0
+    assert wsref.parity_metrics(np.zeros((0, 4)), np.zeros((0, 4))) == (0.0, 0.0)
+    # float32 inputs are compared in FP64: a 1e-9 deviation must not vanish
+    ma, _ = wsref.parity_metrics(np.float64(1.0) + 1e-9, np.float32(1.0))
+    assert abs(ma - 1e-9) < 1e-15
+    # several dimensions: the norm runs over the whole tensor, not per row
+    got, ref = np.zeros((2, 3, 4)), np.zeros((2, 3, 4))
+    ref[0, 0, 0], ref[1, 2, 3], got[1, 2, 3] = 3.0, 4.0, 4.0 + 0.5
+    ma, rf = wsref.parity_metrics(got, ref)
+    assert ma == 3.0 and abs(rf - math.sqrt(9.0 + 0.25) / 5.0) < 1e-15
