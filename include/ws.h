@@ -17,8 +17,14 @@
  *   ws_attn_schedule       host-only diagnostic: the attention work schedule for a given SM count
  *
  * Conventions (all functions)
- *   - Return value: WS_OK (0) or a negative ws_status.  On any error NOTHING is launched and no
- *     output byte is modified.  WS_ERR_CUDA keeps the cudaError_t in ws_last_cuda_error().
+ *   - Return value: WS_OK (0) or a negative ws_status.  Every argument is checked, every TMA
+ *     descriptor encoded and the work schedule built BEFORE the first launch or copy: on any
+ *     argument error (every status except WS_ERR_CUDA) NOTHING is launched, nothing is enqueued
+ *     and no output byte is modified.  WS_ERR_CUDA (the cudaError_t is kept in
+ *     ws_last_cuda_error()) reports a failure of the CUDA runtime itself; if it strikes in the
+ *     middle of a multi-launch call the earlier launches stay enqueued and outputs are undefined.
+ *   - Per-device state (SM count, kernel attributes, a5's helper streams) is keyed by the current
+ *     device: one process may drive several GPUs (cudaSetDevice before the call).
  *   - Pointers documented "device" are CUDA device pointers OWNED BY THE CALLER and borrowed
  *     until the stream-ordered work completes.  Pointers documented "host" are read during the
  *     call only.  Device pointers must be 16-byte aligned and d * sizeof(element) a multiple of
@@ -190,7 +196,9 @@ int ws_block_causal_attn_seq_layout(void* out_seq, float* lse, const void* q_seq
  *   they have landed, and its output returns on a second internal stream.  Both helper streams
  *   (one pair per device, created on first use: the library's only lazily created global state
  *   besides the driver entry point) start after the work already queued on `stream` and are
- *   joined back into it, so to the caller the call is ordered on `stream` like any other.
+ *   joined back into it -- also when a CUDA call fails half way -- so to the caller the call is
+ *   ordered on `stream` like any other and a stream capture is never left unjoined.  Calls on the
+ *   same device from several host threads are serialised for the length of the enqueue.
  *   The call does not synchronise; the caller synchronises the stream before reading out_host.
  *
  *   k_cache, v_cache : device [H, capacity, d]      (the persistent local cache)

@@ -27,19 +27,6 @@
 #include "ws_internal.h"
 #include "ws_ptx.cuh"
 
-#ifdef WS_ATTN_TRACE
-__device__ unsigned long long* g_trace_ptr = nullptr;
-#define WS_TRACE_DECL(role, cond) unsigned long long* trc_ = (blockIdx.x == WS_TRACE_BLOCK && g_trace_ptr && (cond)) ? g_trace_ptr + (role) * 8192 : nullptr; int trc_i_ = 0;
-#define WS_TRACE(ev) do { if (trc_ && trc_i_ < 8190) trc_[trc_i_++] = ((unsigned long long)(ev) << 48) | ((unsigned long long)clock64() & 0xffffffffffffull); } while (0)
-#define WS_TRACE_CTA(slot, ev) do { if (g_trace_ptr && threadIdx.x == (slot) * 32) { unsigned long long gt_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt_)); g_trace_ptr[4 * 8192 + blockIdx.x * 8 + (ev)] = gt_; if ((ev) == 0) { unsigned sm_; asm volatile("mov.u32 %0, %%smid;" : "=r"(sm_)); g_trace_ptr[4 * 8192 + blockIdx.x * 8 + 6] = sm_; } } } while (0)
-#define WS_TRACE_GT(ev) do { if (trc_ && trc_i_ < 8190) { unsigned long long gt_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt_)); trc_[trc_i_++] = ((unsigned long long)(ev) << 48) | (gt_ & 0xffffffffffffull); } } while (0)
-#else
-#define WS_TRACE_GT(ev)
-#define WS_TRACE_CTA(slot, ev)
-#define WS_TRACE_DECL(role, cond)
-#define WS_TRACE(ev)
-#endif
-
 namespace {
 
 constexpr int kBlockM = 128;  // query rows per tile (one TMEM lane each)
@@ -224,7 +211,6 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
   // the warp index goes through a shuffle so that ptxas knows it is warp-uniform: the TMA and MMA
   // warps then run in uniform control flow and their descriptors live in uniform registers
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
-  WS_TRACE_CTA(0, 0);
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < kStages; ++i) {
@@ -254,7 +240,6 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
   __syncthreads();
   ptx::tc_fence_after();
   const uint32_t tmem = bar.tmem_base;
-  WS_TRACE_CTA(0, 1);
   // everything above touched only shared memory, TMEM and the kernel parameters: it overlaps the previous kernel's tail
   wsi::pdl_trigger();
   wsi::pdl_wait();
@@ -324,9 +309,6 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
     } else if (warp == 1) {
       // ============================== MMA issuer ==============================
       uint32_t it = 0, seg = 0, p_phase = 0;
-      WS_TRACE_DECL(0, lane == 0)
-      WS_TRACE(30); WS_TRACE_GT(31);
-      WS_TRACE_CTA(1, 2);
       const uint32_t tmem_u = __shfl_sync(0xffffffffu, tmem, 0);
       // K-major SW128 operand (Q, K): LBO 16 B, SBO 1024 B; MN-major SW128 operand (V): LBO = atom, SBO 1024 B
       constexpr uint64_t kDescK = ((uint64_t)(16 >> 4) << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
@@ -383,21 +365,18 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
           uint32_t it_k = 0, slot_k = 0;
           if (has_next) { it_k = it++; slot_k = it_k % kStages; }
           wait_full(it_v);
-          WS_TRACE(1);
 #pragma unroll
           for (int tile = 0; tile < 2; ++tile) {
 #pragma unroll
             for (int c = 0; c + 1 < kPChunks; ++c) {
               ptx::mbar_wait(ptx::smem_u32(&bar.p_ready[tile][c]), p_phase);
               ptx::tc_fence_after();
-              if (c == 0) WS_TRACE(2 + 4 * tile);
               if (ptx::elect_one()) issue_pv(tile, slot_v, c, acc);
               __syncwarp();
             }
             ptx::mbar_wait(ptx::smem_u32(&bar.p_ready[tile][kPChunks - 1]), p_phase);
             ptx::tc_fence_after();
             if (tile == 0 && has_next) wait_full(it_k);
-            WS_TRACE(3 + 4 * tile);
             if (ptx::elect_one()) {
               issue_pv(tile, slot_v, kPChunks - 1, acc);
               ptx::tc_commit(ptx::smem_u32(&bar.o_done[tile]));
@@ -412,14 +391,11 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
               }
             }
             __syncwarp();
-            WS_TRACE(4 + 4 * tile);
           }
           p_phase ^= 1;
         }
         ++seg;
       }
-      WS_TRACE(32); WS_TRACE_GT(33);
-      WS_TRACE_CTA(1, 3);
     }
   } else {
     // ============================== softmax warpgroups ==============================
@@ -432,7 +408,6 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
     const uint32_t s_full = ptx::smem_u32(&bar.s_full[tile]);
     const uint32_t p_ready = ptx::smem_u32(&bar.p_ready[tile][0]);
     const uint32_t o_done = ptx::smem_u32(&bar.o_done[tile]);
-    WS_TRACE_DECL(1 + tile, (warp & 3) == 0 && lane == 0)
     uint32_t n_iter = 0;  // S tiles consumed so far == PVs requested so far (drives every phase bit)
 
     SegWalk walk(p);
@@ -463,12 +438,10 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
 
         ptx::mbar_wait(s_full, n_iter & 1);
         ptx::tc_fence_after();
-        WS_TRACE(10);
         uint32_t s[4][32];
 #pragma unroll
         for (int q = 0; q < 4; ++q) ptx::tmem_ld32(tS + q * 32, s[q]);
         ptx::tc_wait_ld();
-        WS_TRACE(11);
         if (lim < kBlockN) {
 #pragma unroll
           for (int q = 0; q < 4; ++q)
@@ -509,7 +482,6 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
           }
         }
         const float neg_ms = (m == -INFINITY) ? 0.f : -m * p.scale_log2;
-        WS_TRACE(12);
         // P = 2^(s*scale - m*scale) in kPChunks chunks of 32 keys; each chunk is handed to the MMA warp as soon
         // as it sits in TMEM, so that P.V of the early chunks overlaps the exponentials of the later ones.
         // Tiles in which some row of this warp has masked keys take the all-MUFU variant: ex2(-inf) is
@@ -536,7 +508,6 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
               ptx::tc_wait_st();
               ptx::tc_fence_before();
               ptx::mbar_arrive(p_ready + chunk_ending_at(u + 1) * 8);
-              if (u == 3 || u == 7) WS_TRACE(13 + (u >> 2));
             }
           }
         };
@@ -603,22 +574,20 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
   }
 
   ptx::tc_fence_before();
-  WS_TRACE_CTA(4, 4);
   __syncthreads();
-  WS_TRACE_CTA(0, 5);
   if (warp == 2) ptx::tmem_dealloc(tmem, kTmemCols);
 }
 
 // ---------------------------------------------------------------------------------------------
 // combine kernel: merges the split-KV partials of the phase-2 items, and zero-fills phase-2 items
-// that see no key at all.  grid = (d/4, number of phase-2 items), block = 256 threads (one per row).
+// that see no key at all.  grid = (number of phase-2 items, d/4), block = 256 threads (one per row).
 // ---------------------------------------------------------------------------------------------
 template <int D, bool OUT_F32>
 __global__ void __launch_bounds__(kPairM) attn_combine_kernel(const __grid_constant__ Params p) {
   wsi::pdl_trigger();
   wsi::pdl_wait();  // the partials are the attention kernel's
-  const int w = p.n_waves * p.grid + blockIdx.y, head = w / p.n_pairs, pair = w - head * p.n_pairs;
-  const int q4 = blockIdx.x, r = threadIdx.x;
+  const int w = p.n_waves * p.grid + blockIdx.x, head = w / p.n_pairs, pair = w - head * p.n_pairs;
+  const int q4 = blockIdx.y, r = threadIdx.x;
   const int row = pair * kPairM + r;
   if (row >= p.Lq) return;
   const int Tp = p.pair_prefix[p.n_pairs];
@@ -718,14 +687,45 @@ bool encode_map(CUtensorMap* map, const void* base, uint64_t d0, uint64_t d1, ui
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-int sm_count() {
-  static int n = 0;
-  if (n == 0) {
-    int dev = 0, v = 0;
-    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess)
-      n = v;
+// Per-device state: the SM count and which kernel instantiations already carry their dynamic shared-memory
+// attribute on that device (cudaFuncSetAttribute is per device).  Indexed by cudaGetDevice(), like ws_unit.cu's pipes.
+constexpr int kMaxDevices = 64;
+constexpr int kKernelVariants = 8;
+struct DeviceState {
+  int sms = 0;
+  bool attr_set[kKernelVariants] = {};
+};
+std::mutex g_dev_mu;
+DeviceState g_dev[kMaxDevices];
+
+// The current device's slot with its SM count filled in, or nullptr (no device / index beyond the table).
+DeviceState* device_state(cudaError_t* err) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e == cudaSuccess && (dev < 0 || dev >= kMaxDevices)) e = cudaErrorInvalidDevice;
+  if (e == cudaSuccess) {
+    std::lock_guard<std::mutex> lock(g_dev_mu);
+    DeviceState& st = g_dev[dev];
+    if (st.sms == 0) {
+      int v = 0;
+      e = cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
+      if (e == cudaSuccess && v <= 0) e = cudaErrorNoDevice;
+      if (e == cudaSuccess) st.sms = v;
+    }
+    if (e == cudaSuccess) return &st;
   }
-  return n;
+  if (err) *err = e;
+  return nullptr;
+}
+
+// Sets MaxDynamicSharedMemorySize on `kernel` once per device.
+template <typename K>
+cudaError_t ensure_smem_attr(DeviceState* st, int variant, K kernel, int bytes) {
+  std::lock_guard<std::mutex> lock(g_dev_mu);
+  if (st->attr_set[variant]) return cudaSuccess;
+  const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e == cudaSuccess) st->attr_set[variant] = true;
+  return e;
 }
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
@@ -758,14 +758,10 @@ WsLayout ws_layout(int32_t Lq, int32_t H, int32_t d, int64_t kv_total, int64_t c
 }
 
 template <int D, bool OUT_F32>
-int launch_attention(const Params& prm, cudaStream_t stream) {
+int launch_attention(const Params& prm, DeviceState* st, cudaStream_t stream) {
   using C = Cfg<D>;
-  static std::once_flag once;
-  static cudaError_t attr_err = cudaSuccess;
-  std::call_once(once, [] {
-    attr_err = cudaFuncSetAttribute(attn_fwd_kernel<D, OUT_F32>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes);
-  });
-  if (attr_err != cudaSuccess) return wsi::cuda_fail(attr_err);
+  const cudaError_t ae = ensure_smem_attr(st, (D == 128 ? 0 : 2) + (OUT_F32 ? 1 : 0), attn_fwd_kernel<D, OUT_F32>, C::kSmemBytes);
+  if (ae != cudaSuccess) return wsi::cuda_fail(ae);
   int launches = 0;
   if (prm.grid > 0) {
     const cudaError_t e = wsi::launch_pdl(attn_fwd_kernel<D, OUT_F32>, dim3(prm.grid), dim3(kThreads), C::kSmemBytes, stream, prm);
@@ -774,7 +770,7 @@ int launch_attention(const Params& prm, cudaStream_t stream) {
   }
   const int n_pool_items = prm.H * prm.n_pairs - prm.n_waves * prm.grid;
   if (n_pool_items > 0) {
-    dim3 cgrid(D / 4, (unsigned)n_pool_items);
+    dim3 cgrid((unsigned)n_pool_items, D / 4);  // items on x: H * n_pairs may exceed the 65535 limit of y
     const cudaError_t e = wsi::launch_pdl(attn_combine_kernel<D, OUT_F32>, cgrid, dim3(kPairM), 0, stream, prm);
     if (e != cudaSuccess) return wsi::cuda_fail(e);
     ++launches;
@@ -783,13 +779,6 @@ int launch_attention(const Params& prm, cudaStream_t stream) {
 }
 
 }  // namespace
-
-#ifdef WS_ATTN_TRACE
-extern "C" __attribute__((visibility("default"))) void ws_debug_set_trace(void* p) {
-  unsigned long long* v = reinterpret_cast<unsigned long long*>(p);
-  cudaMemcpyToSymbol(g_trace_ptr, &v, sizeof(v));
-}
-#endif
 
 extern "C" __attribute__((visibility("default"))) size_t ws_block_causal_attn_workspace_bytes(int32_t Lq, int32_t H, int32_t d, int64_t kv_total, ws_dtype dt) {
   if (Lq <= 0 || H <= 0 || d <= 0 || kv_total < 0) return 0;
@@ -897,15 +886,11 @@ extern "C" __attribute__((visibility("default"))) int ws_attn_schedule(int32_t L
   return WS_OK;
 }
 
-namespace {
-// Shared implementation.  q / k_new / v_new / out are token-major with `tok_heads` heads per token in memory, of which
-// the H heads starting at the given base pointers take part (tok_heads == H for the plain [L, H, d] call).
-int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const void* v_cache, int64_t capacity,
-              int64_t cache_len, const void* k_new, const void* v_new, int32_t Ln, int32_t H, int32_t d, int32_t Lq,
-              const ws_block_mask* mask, float softmax_scale, void* workspace, size_t workspace_bytes, ws_dtype dt,
-              void* stream_, int64_t tok_heads) {
-  cudaStream_t stream = (cudaStream_t)stream_;
-  // ---- validation: nothing is launched on any error ----
+// Every argument check of the attention entry points.  Pure host logic: touches no device and launches nothing,
+// so callers that enqueue other work first (ws_unit_forward_host) can run it up front.
+int wsi::attn_validate(const void* out, const float* lse, const void* q, const void* k_cache, const void* v_cache, int64_t capacity,
+                       int64_t cache_len, const void* k_new, const void* v_new, int32_t Ln, int32_t H, int32_t d, int32_t Lq,
+                       const ws_block_mask* mask, float softmax_scale, const void* workspace, size_t workspace_bytes, ws_dtype dt) {
   if (dt != WS_DTYPE_BF16 && dt != WS_DTYPE_F32) return WS_ERR_UNSUPPORTED;
   if (d != 64 && d != 128) return WS_ERR_UNSUPPORTED;
   if (!out || !q || !mask || H <= 0 || Lq <= 0 || Ln < 0 || capacity < 0 || cache_len < 0) return WS_ERR_INVALID_ARG;
@@ -915,43 +900,49 @@ int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const v
   if (cache_len > 0 && (!k_cache || !v_cache)) return WS_ERR_INVALID_ARG;
   if (cache_len + Ln > 0x7fffffffLL / kMaxPairs - kBlockN) return WS_ERR_UNSUPPORTED;  // pair_prefix is int32
   if (const int rc = check_mask(mask, Lq, cache_len, Ln)) return rc;
-  const int n_pairs = (Lq + kPairM - 1) / kPairM;
-  if (n_pairs > kMaxPairs) return WS_ERR_UNSUPPORTED;
+  if ((Lq + kPairM - 1) / kPairM > kMaxPairs) return WS_ERR_UNSUPPORTED;
   if (!wsi::aligned16(out) || !wsi::aligned16(q) || !wsi::aligned16(k_cache) || !wsi::aligned16(v_cache) ||
       !wsi::aligned16(k_new) || !wsi::aligned16(v_new) || (lse && (reinterpret_cast<uintptr_t>(lse) & 3)))
     return WS_ERR_ALIGNMENT;
   const WsLayout L = ws_layout(Lq, H, d, cache_len + Ln, cache_len, Ln, dt, true);
   if (!workspace || workspace_bytes < L.total) return WS_ERR_WORKSPACE;
   if (!wsi::aligned256(workspace)) return WS_ERR_WORKSPACE;
+  return WS_OK;
+}
+
+namespace {
+// Shared implementation.  q / k_new / v_new / out are token-major with `tok_heads` heads per token in memory, of which
+// the H heads starting at the given base pointers take part (tok_heads == H for the plain [L, H, d] call).
+int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const void* v_cache, int64_t capacity,
+              int64_t cache_len, const void* k_new, const void* v_new, int32_t Ln, int32_t H, int32_t d, int32_t Lq,
+              const ws_block_mask* mask, float softmax_scale, void* workspace, size_t workspace_bytes, ws_dtype dt,
+              void* stream_, int64_t tok_heads) {
+  cudaStream_t stream = (cudaStream_t)stream_;
+  // ---- validation, descriptors and schedule first: nothing is launched on any error ----
+  if (const int rc = wsi::attn_validate(out, lse, q, k_cache, v_cache, capacity, cache_len, k_new, v_new, Ln, H, d, Lq, mask,
+                                        softmax_scale, workspace, workspace_bytes, dt))
+    return rc;
+  const int n_pairs = (Lq + kPairM - 1) / kPairM;
+  const WsLayout L = ws_layout(Lq, H, d, cache_len + Ln, cache_len, Ln, dt, true);
   if (!get_encode_fn()) return wsi::cuda_fail(cudaErrorNotSupported);
+  cudaError_t dev_err = cudaErrorNoDevice;
+  DeviceState* dev = device_state(&dev_err);
+  if (!dev) return wsi::cuda_fail(dev_err);
 
   char* ws = reinterpret_cast<char*>(workspace);
-  const void *q_b = q, *kc_b = k_cache, *vc_b = v_cache, *kn_b = k_new, *vn_b = v_new;
-  int64_t cap_b = capacity;
-  int launches = 0;
-  if (dt == WS_DTYPE_F32) {
-    // round the FP32 operands to BF16 on the device (reading R9); the cache copy is compacted to cache_len rows
-    auto cast = [&](void* dstp, const void* srcp, int64_t planes, int64_t plane_elems, int64_t pitch) {
-      const int64_t total = planes * plane_elems;
-      if (total == 0) return;
-      const int blocks = (int)((total + 255) / 256 < 4096 ? (total + 255) / 256 : 4096);
-      (void)wsi::launch_pdl(cast_f32_to_bf16_kernel, dim3(blocks), dim3(256), 0, stream, reinterpret_cast<__nv_bfloat16*>(dstp),
-                            reinterpret_cast<const float*>(srcp), planes, plane_elems, pitch);
-      ++launches;
-    };
-    cast(ws + L.stage_q, q, Lq, (int64_t)H * d, tok_heads * d);  // token by token: the staged copy is compact [Lq, H, d]
-    cast(ws + L.stage_kc, k_cache, H, cache_len * d, capacity * d);
-    cast(ws + L.stage_vc, v_cache, H, cache_len * d, capacity * d);
-    cast(ws + L.stage_kn, k_new, Ln, (int64_t)H * d, tok_heads * d);
-    cast(ws + L.stage_vn, v_new, Ln, (int64_t)H * d, tok_heads * d);
-    q_b = ws + L.stage_q; kc_b = ws + L.stage_kc; vc_b = ws + L.stage_vc; kn_b = ws + L.stage_kn; vn_b = ws + L.stage_vn;
-    cap_b = cache_len;
-  }
+  const bool f32 = dt == WS_DTYPE_F32;
+  // WS_DTYPE_F32 (reading R9): the kernel reads BF16 copies staged in the workspace; the cache copy is compacted to cache_len rows
+  const void* q_b = f32 ? ws + L.stage_q : q;
+  const void* kc_b = f32 ? ws + L.stage_kc : k_cache;
+  const void* vc_b = f32 ? ws + L.stage_vc : v_cache;
+  const void* kn_b = f32 ? ws + L.stage_kn : k_new;
+  const void* vn_b = f32 ? ws + L.stage_vn : v_new;
+  const int64_t cap_b = f32 ? cache_len : capacity;
 
   Params prm;
   memset(&prm, 0, sizeof(prm));
   const uint64_t row_b = (uint64_t)d * 2;
-  const uint64_t tok_b = row_b * (uint64_t)(dt == WS_DTYPE_F32 ? H : tok_heads);  // token pitch of the BF16 operands
+  const uint64_t tok_b = row_b * (uint64_t)(f32 ? H : tok_heads);  // token pitch of the BF16 operands
   bool ok = encode_map(&prm.map_q, q_b, d, H, Lq, row_b, tok_b, 1, kBlockM);
   // a source with no rows still needs a well-formed (never dereferenced) descriptor
   ok = ok && (Ln > 0 ? encode_map(&prm.map_kn, kn_b, d, H, Ln, row_b, tok_b, 1, kBlockN)
@@ -979,15 +970,31 @@ int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const v
     prm.kv_visible[b] = mask->kv_visible[b];
   }
   const int64_t Tp = build_pair_prefix(prm, mask, Lq, cache_len);
-  {
-    const int sms = sm_count();
-    if (sms <= 0) return wsi::cuda_fail(cudaErrorNoDevice);
-    build_schedule(prm, Tp, sms);
+  build_schedule(prm, Tp, dev->sms);
+
+  // ---- launches ----
+  if (f32) {
+    int launches = 0;
+    cudaError_t ce = cudaSuccess;
+    auto cast = [&](const void* dstp, const void* srcp, int64_t planes, int64_t plane_elems, int64_t pitch) {
+      const int64_t total = planes * plane_elems;
+      if (total == 0 || ce != cudaSuccess) return;
+      const int blocks = (int)((total + 255) / 256 < 4096 ? (total + 255) / 256 : 4096);
+      ce = wsi::launch_pdl(cast_f32_to_bf16_kernel, dim3(blocks), dim3(256), 0, stream,
+                           reinterpret_cast<__nv_bfloat16*>(const_cast<void*>(dstp)), reinterpret_cast<const float*>(srcp), planes,
+                           plane_elems, pitch);
+      if (ce == cudaSuccess) ++launches;
+    };
+    cast(q_b, q, Lq, (int64_t)H * d, tok_heads * d);  // token by token: the staged copy is compact [Lq, H, d]
+    cast(kc_b, k_cache, H, cache_len * d, capacity * d);
+    cast(vc_b, v_cache, H, cache_len * d, capacity * d);
+    cast(kn_b, k_new, Ln, (int64_t)H * d, tok_heads * d);
+    cast(vn_b, v_new, Ln, (int64_t)H * d, tok_heads * d);
+    if (launches) wsi::count_launch(launches);
+    if (ce != cudaSuccess) return wsi::cuda_fail(ce);
   }
-  if (launches) wsi::count_launch(launches);
-  const bool f32 = dt == WS_DTYPE_F32;
-  if (d == 128) return f32 ? launch_attention<128, true>(prm, stream) : launch_attention<128, false>(prm, stream);
-  return f32 ? launch_attention<64, true>(prm, stream) : launch_attention<64, false>(prm, stream);
+  if (d == 128) return f32 ? launch_attention<128, true>(prm, dev, stream) : launch_attention<128, false>(prm, dev, stream);
+  return f32 ? launch_attention<64, true>(prm, dev, stream) : launch_attention<64, false>(prm, dev, stream);
 }
 }  // namespace
 

@@ -136,9 +136,9 @@ int relayout(void* const* dsts, const void* const* srcs, int n_tensors, int64_t 
 
 }  // namespace
 
-extern "C" __attribute__((visibility("default"))) int ws_kv_cache_write(void* k_cache, void* v_cache, int64_t capacity, int32_t H, int32_t d, const void* k_src,
-                                 const void* v_src, int32_t n_rows, int32_t H_src, int32_t head_begin, int64_t row_offset,
-                                 ws_dtype dt, void* stream) {
+// Every argument check of ws_kv_cache_write (host only; see ws_internal.h).
+int wsi::cache_write_validate(const void* k_cache, const void* v_cache, int64_t capacity, int32_t H, int32_t d, const void* k_src,
+                              const void* v_src, int32_t n_rows, int32_t H_src, int32_t head_begin, int64_t row_offset, ws_dtype dt) {
   const int es = wsi::elem_bytes(dt);
   if (es == 0) return WS_ERR_UNSUPPORTED;
   if (!k_cache || !v_cache || capacity <= 0 || H <= 0 || d <= 0 || n_rows < 0 || H_src <= 0 || head_begin < 0 ||
@@ -150,6 +150,7 @@ extern "C" __attribute__((visibility("default"))) int ws_kv_cache_write(void* k_
   if (row_bytes % 16 != 0 || !wsi::aligned16(k_cache) || !wsi::aligned16(v_cache) || !wsi::aligned16(k_src) ||
       !wsi::aligned16(v_src))
     return WS_ERR_ALIGNMENT;
+  if (H > 65535 || row_bytes / 16 > (1 << 20)) return WS_ERR_UNSUPPORTED;  // launch_copy's limits
   if (n_rows == 0) return WS_OK;
   const size_t cache_bytes = (size_t)H * capacity * row_bytes, src_bytes = (size_t)n_rows * H_src * row_bytes;
   const void* caches[2] = {k_cache, v_cache};
@@ -158,6 +159,16 @@ extern "C" __attribute__((visibility("default"))) int ws_kv_cache_write(void* k_
     for (int j = 0; j < 2; ++j)
       if (wsi::ranges_overlap(caches[i], cache_bytes, srcs[j], src_bytes)) return WS_ERR_OVERLAP;
   if (wsi::ranges_overlap(k_cache, cache_bytes, v_cache, cache_bytes)) return WS_ERR_OVERLAP;
+  return WS_OK;
+}
+
+extern "C" __attribute__((visibility("default"))) int ws_kv_cache_write(void* k_cache, void* v_cache, int64_t capacity, int32_t H, int32_t d, const void* k_src,
+                                 const void* v_src, int32_t n_rows, int32_t H_src, int32_t head_begin, int64_t row_offset,
+                                 ws_dtype dt, void* stream) {
+  if (const int rc = wsi::cache_write_validate(k_cache, v_cache, capacity, H, d, k_src, v_src, n_rows, H_src, head_begin, row_offset, dt))
+    return rc;
+  if (n_rows == 0) return WS_OK;
+  const int64_t row_bytes = (int64_t)d * wsi::elem_bytes(dt);
   const int64_t dv = row_bytes / 16;
   // a = head h, b = row r:  src (r * H_src + head_begin + h) * dv ; dst (h * capacity + row_offset + r) * dv
   const char* ks = reinterpret_cast<const char*>(k_src) + (int64_t)head_begin * row_bytes;

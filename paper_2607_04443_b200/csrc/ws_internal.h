@@ -21,6 +21,14 @@ inline bool ranges_overlap(const void* a, size_t na, const void* b, size_t nb) {
   return na != 0 && nb != 0 && a0 < b0 + nb && b0 < a0 + na;
 }
 
+// Host-only argument checks of ws_block_causal_attn (ws_attn.cu) and ws_kv_cache_write (ws_copy.cu): no device is
+// touched and nothing is launched, so a composite entry point can run them before it enqueues anything.
+int attn_validate(const void* out, const float* lse, const void* q, const void* k_cache, const void* v_cache, int64_t capacity,
+                  int64_t cache_len, const void* k_new, const void* v_new, int32_t Ln, int32_t H, int32_t d, int32_t Lq,
+                  const ws_block_mask* mask, float softmax_scale, const void* workspace, size_t workspace_bytes, ws_dtype dt);
+int cache_write_validate(const void* k_cache, const void* v_cache, int64_t capacity, int32_t H, int32_t d, const void* k_src,
+                         const void* v_src, int32_t n_rows, int32_t H_src, int32_t head_begin, int64_t row_offset, ws_dtype dt);
+
 // After a launch: pick up launch-configuration errors without synchronising.
 inline int after_launch(int n_launches) {
   cudaError_t e = cudaPeekAtLastError();

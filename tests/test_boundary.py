@@ -122,6 +122,54 @@ def test_attention_rejects_bad_arguments(lib):
     assert call(qe=tuple(range(1, 131)), kv=tuple([576] * 130), Lq=130) == UNSUPPORTED  # > WS_MAX_MASK_BLOCKS
 
 
+def test_unit_forward_host_checks_everything_before_enqueueing(lib):
+    """ws_unit_forward_host runs every check of the calls it is made of (cache write, attention) up front, so a call
+    that will fail enqueues no copy and forks no helper stream.  On this CPU-only box that is observable: every
+    argument error comes back as itself, never as WS_ERR_CUDA from a first CUDA call."""
+    f = lib.ws_unit_forward_host
+    sb = lib.ws_unit_forward_host_staging_bytes
+
+    def call(out=0x1000, q=0x2000, kn=0x3000, vn=0x4000, Lq=300, Ln=300, steps=2, kc=A, vc=B, cap=4096, ks=0x5000, vs=0x6000, n=100,
+             off=500, Tc=600, H=8, d=64, scale=0.125, st=0x70000000, stb=None):
+        need = sb(Lq, Ln, H, d, n, Tc + Ln, steps) if (Lq > 0 and steps > 0 and H > 0 and Tc + Ln >= 0 and n >= 0 and Ln >= 0) else 0
+        return f(P(out), P(q), P(kn) if kn else None, P(vn) if vn else None, Lq, Ln, steps, P(kc), P(vc), cap, P(ks) if ks else None,
+                 P(vs) if vs else None, n, off, Tc, H, d, scale, P(st) if st else None, need if stb is None else stb, None)
+
+    assert call(kc=A + 8) == ALIGN                  # misaligned cache pointer: found by the cache-write / attention checks
+    assert call(vc=B + 2) == ALIGN
+    assert call(Lq=256 * 256 + 1, Ln=0, kn=0, vn=0) == UNSUPPORTED   # more than 256 Q-tile pairs
+    assert call(cap=1 << 24, Tc=(0x7fffffff // 256), n=0, ks=0, vs=0, off=0) == UNSUPPORTED  # beyond the attention kernel's key limit
+    assert call(scale=float("nan")) == INVALID
+    assert call(scale=-0.5) == INVALID
+    assert call(vc=A + 4096) == OVERLAP             # K and V cache ranges intersect
+    assert call(kc=0x70000000) == OVERLAP           # staging (where the slice lands) inside the K cache
+    assert call(off=4096 - 99) == RANGE
+    assert call(Tc=4097) == RANGE
+    assert call(d=96) == UNSUPPORTED
+    assert call(kn=0) == INVALID
+    assert call(ks=0) == INVALID
+    assert call(st=0) == WORKSPACE
+    assert call(st=0x70000010) == WORKSPACE
+    assert call(stb=4096) == WORKSPACE
+    assert call(steps=0) == INVALID
+    if not torch.cuda.is_available():
+        assert call() == CUDA                       # a valid call reaches CUDA and fails there: no CPU fallback
+
+
+def test_attention_accepts_more_than_65535_work_items(lib):
+    """H * ceil(Lq / 256) above 65535 used to overflow the combine kernel's gridDim.y after the attention kernel had
+    already run; the item index now sits on gridDim.x.  The schedule for such a problem must build."""
+    n_sms = 148
+    grid, n_waves = ctypes.c_int32(), ctypes.c_int32()
+    tiles = (ctypes.c_int32 * 4)()
+    pool = (ctypes.c_int64 * (n_sms + 1))()
+    Mask = binding._BlockMask
+    m = Mask(1, (ctypes.c_int32 * 1)(520), (ctypes.c_int32 * 1)(300))
+    H = 40000  # x 3 pairs = 120000 items
+    assert lib.ws_attn_schedule(520, H, 300, 0, ctypes.byref(m), n_sms, ctypes.byref(grid), ctypes.byref(n_waves), tiles, pool) == OK
+    assert grid.value == n_sms and n_waves.value == (H * 3) // n_sms
+
+
 def test_workspace_bytes_is_sane(lib):
     f = lib.ws_block_causal_attn_workspace_bytes
     assert f(0, 1, 128, 10, 0) == 0

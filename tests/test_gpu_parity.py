@@ -593,3 +593,22 @@ def test_fused_relayout_attention_in_fp32():
                                            np.ascontiguousarray(vn[:, sel]), qe, kv, scale)
     check_attn(got[:, sel], ref, lse.cpu().numpy(), ref_lse, what="fused fp32")
     assert np.all(got[:, :g0 * Hp] == 5.0), "heads of other ranks must not be touched"
+
+
+def test_per_device_state_survives_device_round_trips():
+    """The SM count and the kernels' shared-memory attribute are kept per device (ws.h conventions): the library is
+    called on every visible device in turn, twice, each time after a cudaSetDevice; on a one-GPU box this walks the
+    per-device table path for device 0 after set_device round trips."""
+    c = rand_case(41, 3, 128, [300], [700], 500, 200)
+    ref, _ = wsref.block_causal_attn(c["q"], c["k_cache"], c["v_cache"], c["cache_len"], c["k_new"], c["v_new"], c["q_block_end"],
+                                     c["kv_visible"], c["scale"])
+    n_dev = torch.cuda.device_count()
+    try:
+        for _ in range(2):
+            for dev in range(n_dev):
+                torch.cuda.set_device(dev)
+                got, _ = gpu_attention(c["q"], c["k_cache"], c["v_cache"], c["cache_len"], c["k_new"], c["v_new"], c["q_block_end"],
+                                       c["kv_visible"], c["scale"])
+                check_attn(got, ref, what=f"device {dev}")
+    finally:
+        torch.cuda.set_device(0)
