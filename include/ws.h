@@ -220,14 +220,18 @@ int ws_unit_forward_host(void* out_host, const void* q_host, const void* k_new_h
                          size_t staging_bytes, void* stream);
 
 /* Host-only diagnostic (touches no device): the work schedule ws_block_causal_attn would use for this problem on
- * a device with n_sms SMs ("Schedule").  Work item i = head * n_pairs + pair, n_pairs =
- * ceil(Lq / 256); pair p has pair_tiles[p] KV-tile iterations.  CTA c < *grid runs the whole items w * grid + c
- * for w < *n_waves, then the flattened iterations [pool_begin[c], pool_begin[c + 1]) of the remaining items
- * (coordinate of item i, tile j: (i / n_pairs) * sum(pair_tiles) + sum(pair_tiles[0 .. i % n_pairs)) + j).
- *   pair_tiles : host, >= ceil(Lq / 256) entries (written);  pool_begin : host, >= n_sms + 1 entries (written)
+ * a device with n_sms SMs ("Schedule").  The Q rows of a head are cut into 128-row tiles; tiles
+ * (2u, 2u + 1) form PAIR unit u, which runs one iteration per KV tile (unit_kv_tiles[u] of them: what the later
+ * tile's last row sees), both tiles on the same KV tile; an odd last tile is a SINGLE unit whose unit_kv_tiles[u]
+ * KV tiles are walked two per iteration (unit_iters[u] = ceil(unit_kv_tiles[u] / 2)).  Work item i =
+ * head * n_units + unit, n_units = ceil(Lq / 256).  CTA c < *grid runs the whole items w * grid + c for
+ * w < *n_waves, then the flattened iterations [pool_begin[c], pool_begin[c + 1]) of the remaining items
+ * (coordinate of item i, iteration k: (i / n_units) * sum(unit_iters) + sum(unit_iters[0 .. i % n_units)) + k).
+ * Iterations [i0, i1) of a single unit cover its KV tiles [2 i0, min(2 i1, unit_kv_tiles)).
+ *   unit_iters, unit_kv_tiles : host, >= ceil(Lq / 256) entries (written);  pool_begin : host, >= n_sms + 1 entries
  * Errors: INVALID_ARG, OUT_OF_RANGE, UNSUPPORTED as for the mask of ws_block_causal_attn. */
 int ws_attn_schedule(int32_t Lq, int32_t H, int64_t cache_len, int32_t Ln, const ws_block_mask* mask, int32_t n_sms,
-                     int32_t* grid, int32_t* n_waves, int32_t* pair_tiles, int64_t* pool_begin);
+                     int32_t* grid, int32_t* n_waves, int32_t* unit_iters, int32_t* unit_kv_tiles, int64_t* pool_begin);
 
 /* ---- utilities ---- */
 const char* ws_status_string(int status); /* static string, never NULL */

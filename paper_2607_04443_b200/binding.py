@@ -76,7 +76,7 @@ def load():
                                          vp, sz, vp]
     lib.ws_unit_forward_host.restype = ctypes.c_int
     lib.ws_attn_schedule.argtypes = [i32, i32, i64, i32, ctypes.POINTER(_BlockMask), i32, ctypes.POINTER(i32), ctypes.POINTER(i32),
-                                     ctypes.POINTER(i32), ctypes.POINTER(i64)]
+                                     ctypes.POINTER(i32), ctypes.POINTER(i32), ctypes.POINTER(i64)]
     lib.ws_attn_schedule.restype = ctypes.c_int
     lib.ws_status_string.argtypes = [ctypes.c_int]
     lib.ws_status_string.restype = ctypes.c_char_p
@@ -267,18 +267,21 @@ def block_causal_attn_seq_layout(out_seq, q_seq, k_cache, v_cache, cache_len: in
 
 def attn_schedule(Lq: int, H: int, cache_len: int, Ln: int, q_block_end: Sequence[int], kv_visible: Sequence[int], n_sms: int):
     """Host-only: the attention work schedule for a device with n_sms SMs (ws.h ws_attn_schedule).
-    Returns dict(grid, n_waves, pair_tiles [n_pairs], pool_begin [grid + 1])."""
+    Returns dict(grid, n_waves, unit_iters [n_units], unit_kv_tiles [n_units], pool_begin [grid + 1])."""
     n = len(q_block_end)
     qe = (ctypes.c_int32 * n)(*[int(x) for x in q_block_end])
     kv = (ctypes.c_int32 * n)(*[int(x) for x in kv_visible])
     mask = _BlockMask(n, qe, kv)
-    n_pairs = (Lq + 255) // 256
+    n_units = (Lq + 255) // 256
     grid, waves = ctypes.c_int32(0), ctypes.c_int32(0)
-    tiles = (ctypes.c_int32 * max(n_pairs, 1))()
+    iters = (ctypes.c_int32 * max(n_units, 1))()
+    tiles = (ctypes.c_int32 * max(n_units, 1))()
     pool = (ctypes.c_int64 * (n_sms + 1))()
-    rc = load().ws_attn_schedule(Lq, H, int(cache_len), Ln, ctypes.byref(mask), n_sms, ctypes.byref(grid), ctypes.byref(waves), tiles, pool)
+    rc = load().ws_attn_schedule(Lq, H, int(cache_len), Ln, ctypes.byref(mask), n_sms, ctypes.byref(grid), ctypes.byref(waves), iters,
+                                 tiles, pool)
     _ok(rc, "ws_attn_schedule")
-    return dict(grid=grid.value, n_waves=waves.value, pair_tiles=list(tiles)[:n_pairs], pool_begin=list(pool)[:grid.value + 1])
+    return dict(grid=grid.value, n_waves=waves.value, unit_iters=list(iters)[:n_units], unit_kv_tiles=list(tiles)[:n_units],
+                pool_begin=list(pool)[:grid.value + 1])
 
 
 def unit_forward_host_staging_bytes(Lq, Ln, H, d, n_slice_rows, kv_total, n_steps) -> int:

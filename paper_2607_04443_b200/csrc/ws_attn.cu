@@ -9,11 +9,16 @@
 //   * the online softmax is done by two 128-thread warpgroups, one per Q tile, one thread per
 //     query row (tcgen05.ld 32x32b gives each thread its row: no shuffles), exp2 with the scale
 //     folded in, and a lazy rescale of O (only when the running max grows by more than 2^8);
-//   * block-causality is exploited at tile level: a Q-tile pair only visits the KV tiles its
+//   * block-causality is exploited at tile level: a unit of work only visits the KV tiles its
 //     last row can see, and only boundary tiles pay for per-row column masking;
-//   * a persistent stream-K schedule splits the flattened (head, Q-pair, KV-tile) iteration space
-//     evenly over one CTA per SM; a segment that does not cover its whole KV range writes an
-//     FP32 partial (O, m, l) and a small combine kernel merges the partials.
+//   * a CTA has two tile slots (S/P/O sets in TMEM, one softmax warpgroup each) that ping-pong on the
+//     tensor pipe.  A work unit is either a PAIR of consecutive 128-row Q tiles of one head (both slots
+//     walk the same KV tiles and share each K/V tile in shared memory) or, for the ragged last Q tile of
+//     a head, a SINGLE tile whose KV range is cut in two halves, one per slot (the two partial results
+//     are merged inside the CTA through TMEM), so a tail tile costs half a pair instead of a whole one;
+//   * a persistent stream-K schedule splits the flattened (head, unit, iteration) space evenly over
+//     one CTA per SM; a segment that does not cover its unit's whole KV range writes FP32 partials
+//     (O, m, l) and a small combine kernel merges them.
 //
 // Roofline: tensor pipe.  Algorithmic flops = 4 * d * H * sum_b |block b| * kv_visible[b].
 #include <cuda.h>
@@ -59,7 +64,7 @@ __host__ __device__ constexpr int chunk_ending_at(int u) {
 }
 static_assert(chunk16(0) == 0 && chunk16(kPChunks) == 8, "chunks cover the 128 keys of a tile");
 constexpr int kThreads = 384; // warp 0 TMA, warp 1 MMA, warp 2 TMEM alloc, warp 3 idle, warps 4-7 / 8-11 softmax
-constexpr int kMaxPairs = 256;
+constexpr int kMaxUnits = 256;  // work units (Q-tile pairs, plus one single tile) per head
 constexpr int kMaxCtas = 256; // upper bound on the persistent grid (workspace sizing)
 constexpr int kTmemCols = 512;
 constexpr float kLog2e = 1.4426950408889634f;
@@ -68,26 +73,34 @@ constexpr float kRescaleThreshold = 8.0f;  // log2 units: P stays below 2^8
 #ifndef WS_POLY_OF4
 #define WS_POLY_OF4 1
 #endif
-constexpr int kPolyOf4 = WS_POLY_OF4;  // of every 4 pairs of exponentials, this many run on the FMA pipe instead of MUFU
+constexpr int kPolyOf4 = WS_POLY_OF4;
+#ifndef WS_WARP_ARRIVE
+#define WS_WARP_ARRIVE 0
+#endif
+constexpr int kPReadyArrivals = WS_WARP_ARRIVE ? 4 : 128;  // arrivals per P-chunk barrier: one per softmax warp, or one per thread  // of every 4 pairs of exponentials, this many run on the FMA pipe instead of MUFU
 
 struct alignas(64) Params {
   CUtensorMap map_q, map_kn, map_vn, map_kc, map_vc;
   void* out;
   float* lse;
-  float* part_o;   // [slots][d/4][256][4]
-  float2* part_ml; // [slots][256] (m * scale * log2e, l)
+  float* part_o;   // [records][d/4][128][4]
+  float2* part_ml; // [records][128] (m * scale * log2e, l)
   int64_t cache_len;
   int64_t out_pitch;  // elements between consecutive tokens of `out` (H * d, or H_total * d for the token-major rank view)
-  int32_t Lq, H, Ln, n_blocks, n_pairs, n_cache_tiles;
+  int32_t Lq, H, Ln, n_blocks, n_units, n_cache_tiles;
+  // the last unit of a head is a single Q tile (odd number of Q tiles) that sees last_kv_tiles KV tiles
+  int32_t last_single, last_kv_tiles;
   float scale, scale_log2;
   int32_t q_block_end[WS_MAX_MASK_BLOCKS];
   int32_t kv_visible[WS_MAX_MASK_BLOCKS];
-  int32_t pair_prefix[kMaxPairs + 1];  // KV-tile iterations before Q-tile pair p (per head); host-built schedule
-  // Two-phase schedule (host-built).  Work item i = head * n_pairs + pair.  Phase 1: CTA c runs the whole
-  // items w * grid + c, w < n_waves (no partials; the pairs of one head start together on neighbouring
-  // CTAs, so a K/V tile is fetched from DRAM once and hit in L2 by the other pairs).  Phase 2: the
-  // remaining items [n_waves * grid, H * n_pairs) are split stream-K style, CTA c taking the flattened
-  // KV-tile iterations [pool_begin[c], pool_begin[c + 1]) (global coordinates head * Tp + pair_prefix).
+  // unit_prefix[u]: CTA iterations before unit u (per head); host-built.  A pair unit takes one iteration per KV
+  // tile its later Q tile can see; a single unit takes one iteration per TWO KV tiles (one per slot).
+  int32_t unit_prefix[kMaxUnits + 1];
+  // Two-phase schedule (host-built).  Work item i = head * n_units + unit.  Phase 1: CTA c runs the whole
+  // items w * grid + c, w < n_waves (no partials; the units of one head start together on neighbouring
+  // CTAs, so a K/V tile is fetched from DRAM once and hit in L2 by the others).  Phase 2: the
+  // remaining items [n_waves * grid, H * n_units) are split stream-K style, CTA c taking the flattened
+  // iterations [pool_begin[c], pool_begin[c + 1]) (global coordinates head * Tp + unit_prefix).
   int32_t n_waves, grid;
   int64_t pool_begin[kMaxCtas + 1];
 };
@@ -105,11 +118,11 @@ __device__ __forceinline__ int block_of_row(const Params& p, int row) {
   return lo;
 }
 
-__device__ __forceinline__ int pair_of_iter(const Params& s, int n_pairs, int rem) {
-  int lo = 0, hi = n_pairs - 1;  // largest p with pair_prefix[p] <= rem
+__device__ __forceinline__ int unit_of_iter(const Params& s, int rem) {
+  int lo = 0, hi = s.n_units - 1;  // largest u with unit_prefix[u] <= rem
   while (lo < hi) {
     const int mid = (lo + hi + 1) >> 1;
-    if (s.pair_prefix[mid] <= rem) lo = mid; else hi = mid - 1;
+    if (s.unit_prefix[mid] <= rem) lo = mid; else hi = mid - 1;
   }
   return lo;
 }
@@ -125,28 +138,27 @@ __device__ __forceinline__ int cta_of_iter(const Params& p, int64_t t) {
 }
 
 struct Segment {
-  int head, pair, j0, j1, n_tiles;  // KV tiles [j0, j1) of the pair's n_tiles
+  int head, unit, i0, i1, n_iters;  // iterations [i0, i1) of the unit's n_iters
 };
 
 // Walks the CTA's phase-2 share [t, hi) of the flattened iteration space.
 __device__ __forceinline__ Segment next_pool_segment(const Params& p, int64_t& t, int64_t hi) {
-  const Params& s = p;
-  const int Tp = s.pair_prefix[p.n_pairs];
+  const int Tp = p.unit_prefix[p.n_units];
   Segment g;
   g.head = (int)(t / Tp);
   const int rem = (int)(t - (int64_t)g.head * Tp);
-  g.pair = pair_of_iter(s, p.n_pairs, rem);
-  g.n_tiles = s.pair_prefix[g.pair + 1] - s.pair_prefix[g.pair];
-  g.j0 = rem - s.pair_prefix[g.pair];
+  g.unit = unit_of_iter(p, rem);
+  g.n_iters = p.unit_prefix[g.unit + 1] - p.unit_prefix[g.unit];
+  g.i0 = rem - p.unit_prefix[g.unit];
   const int64_t left = hi - t;
-  g.j1 = (int)min((int64_t)g.n_tiles, g.j0 + left);
-  t += g.j1 - g.j0;
+  g.i1 = (int)min((int64_t)g.n_iters, g.i0 + left);
+  t += g.i1 - g.i0;
   return g;
 }
 
 // A CTA's walk over its segments: whole items first (phase 1), then its stream-K range (phase 2).
-// Every role of the CTA runs the same walk, so they agree on the segment sequence.  An item that
-// sees no key at all is reported with n_tiles == 0 (phase 1 only): the softmax warps zero-fill its
+// Every role of the CTA runs the same walk, so they agree on the segment sequence.  A unit that
+// sees no key at all is reported with n_iters == 0 (phase 1 only): the softmax warps zero-fill its
 // rows, the TMA and MMA warps skip it.
 struct SegWalk {
   int wave;
@@ -156,11 +168,11 @@ struct SegWalk {
     if (wave < p.n_waves) {
       const int item = wave * p.grid + (int)blockIdx.x;
       ++wave;
-      g.head = item / p.n_pairs;
-      g.pair = item - g.head * p.n_pairs;
-      g.n_tiles = p.pair_prefix[g.pair + 1] - p.pair_prefix[g.pair];
-      g.j0 = 0;
-      g.j1 = g.n_tiles;
+      g.head = item / p.n_units;
+      g.unit = item - g.head * p.n_units;
+      g.n_iters = p.unit_prefix[g.unit + 1] - p.unit_prefix[g.unit];
+      g.i0 = 0;
+      g.i1 = g.n_iters;
       return true;
     }
     if (t < hi) {
@@ -170,6 +182,32 @@ struct SegWalk {
     return false;
   }
 };
+
+// What the two tile slots of the CTA do in a segment.  Slot s runs Q tile q_tile[s] against the KV tiles
+// jb[s], jb[s] + 1, ... for n_it iterations.  Pair: both slots walk the same KV tiles (shared K/V tiles in shared
+// memory).  Single: the segment's KV tiles [2 i0, min(2 i1, n)) are cut in two runs of n_it tiles; a run that
+// reaches past the visible range computes fully masked tiles (TMA zero fill beyond the tensors), which contribute
+// nothing.
+struct SlotPlan {
+  int q_tile[2], jb[2], n_it;
+  bool single, whole;  // whole: the segment covers the unit's entire KV range
+};
+__device__ __forceinline__ SlotPlan plan_of(const Params& p, const Segment& g) {
+  SlotPlan sp;
+  sp.single = p.last_single && g.unit == p.n_units - 1;
+  sp.whole = g.i0 == 0 && g.i1 == g.n_iters;
+  sp.n_it = g.i1 - g.i0;
+  sp.q_tile[0] = 2 * g.unit;
+  if (sp.single) {
+    sp.q_tile[1] = 2 * g.unit;
+    sp.jb[0] = 2 * g.i0;
+    sp.jb[1] = 2 * g.i0 + sp.n_it;
+  } else {
+    sp.q_tile[1] = 2 * g.unit + 1;
+    sp.jb[0] = sp.jb[1] = g.i0;
+  }
+  return sp;
+}
 
 // ---------------------------------------------------------------------------------------------
 // the attention kernel
@@ -181,7 +219,8 @@ struct Cfg {
   static constexpr int kTileBytes = kAtoms * kAtomBytes;  // one Q tile == one K or V tile
   static constexpr int kSmemQ = 2 * kTileBytes;
   static constexpr int kSmemKV = kStages * kTileBytes;
-  static constexpr int kSmemBytes = kSmemQ + kSmemKV + 256 /*barriers*/;
+  static constexpr int kSmemMerge = kBlockM * 8;           // (m, l) of slot 1 for the in-CTA merge of a single unit
+  static constexpr int kSmemBytes = kSmemQ + kSmemKV + 256 /*barriers*/ + kSmemMerge;
   static_assert(kSmemBytes <= 227 * 1024, "shared memory budget");
   static constexpr uint32_t kTmemS0 = 0, kTmemS1 = 128, kTmemO0 = 256, kTmemO1 = 256 + D;
   static constexpr uint32_t kIdescQK = ptx::make_idesc_bf16(kBlockM, kBlockN, false);
@@ -207,6 +246,7 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
   const uint32_t sKV = smem_base + C::kSmemQ;
   Barriers& bar = *reinterpret_cast<Barriers*>(smem + C::kSmemQ + C::kSmemKV);
   static_assert(sizeof(Barriers) <= 256, "barrier block");
+  float2* merge_ml = reinterpret_cast<float2*>(smem + C::kSmemQ + C::kSmemKV + 256);
 
   // the warp index goes through a shuffle so that ptxas knows it is warp-uniform: the TMA and MMA
   // warps then run in uniform control flow and their descriptors live in uniform registers
@@ -221,7 +261,7 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
     ptx::mbar_init(ptx::smem_u32(&bar.q_empty), 1);
     for (int t = 0; t < 2; ++t) {
       ptx::mbar_init(ptx::smem_u32(&bar.s_full[t]), 1);
-      for (int c = 0; c < kPChunks; ++c) ptx::mbar_init(ptx::smem_u32(&bar.p_ready[t][c]), kBlockM);
+      for (int c = 0; c < kPChunks; ++c) ptx::mbar_init(ptx::smem_u32(&bar.p_ready[t][c]), kPReadyArrivals);
       ptx::mbar_init(ptx::smem_u32(&bar.o_done[t]), 1);
     }
     ptx::fence_mbar_init();
@@ -252,17 +292,19 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
     // register->uniform-register waterfall loop (measured: ~100 cycles of issue per MMA).
     auto bcast_segment = [&](Segment g) {
       g.head = __shfl_sync(0xffffffffu, g.head, 0);
-      g.pair = __shfl_sync(0xffffffffu, g.pair, 0);
-      g.j0 = __shfl_sync(0xffffffffu, g.j0, 0);
-      g.j1 = __shfl_sync(0xffffffffu, g.j1, 0);
-      g.n_tiles = __shfl_sync(0xffffffffu, g.n_tiles, 0);
+      g.unit = __shfl_sync(0xffffffffu, g.unit, 0);
+      g.i0 = __shfl_sync(0xffffffffu, g.i0, 0);
+      g.i1 = __shfl_sync(0xffffffffu, g.i1, 0);
+      g.n_iters = __shfl_sync(0xffffffffu, g.n_iters, 0);
       return g;
     };
     const int n_cache_tiles = p.n_cache_tiles;
     if (warp == 0) {
       // ============================== TMA producer ==============================
+      // Ring order per segment: K of iteration 0 (one tile, or one per slot when the slots walk different KV
+      // tiles), then per iteration V (one or two), K of the next iteration (one or two).
       uint32_t it = 0, seg = 0;
-      auto load_kv = [&](const Segment& g, int j, bool is_v) {
+      auto load_kv = [&](int head, int j, bool is_v) {
         const uint32_t slot = it % kStages, ph = (it / kStages) & 1;
         ptx::mbar_wait(ptx::smem_u32(&bar.kv_empty[slot]), ph ^ 1);
         const uint32_t full = ptx::smem_u32(&bar.kv_full[slot]);
@@ -272,12 +314,12 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
           if (j < n_cache_tiles) {
             const void* map = is_v ? (const void*)&p.map_vc : (const void*)&p.map_kc;
 #pragma unroll
-            for (int a = 0; a < C::kAtoms; ++a) ptx::tma_load_3d(dst + a * C::kAtomBytes, map, full, a * 64, j * kBlockN, g.head);
+            for (int a = 0; a < C::kAtoms; ++a) ptx::tma_load_3d(dst + a * C::kAtomBytes, map, full, a * 64, j * kBlockN, head);
           } else {
             const void* map = is_v ? (const void*)&p.map_vn : (const void*)&p.map_kn;
             const int r0 = (j - n_cache_tiles) * kBlockN;
 #pragma unroll
-            for (int a = 0; a < C::kAtoms; ++a) ptx::tma_load_3d(dst + a * C::kAtomBytes, map, full, a * 64, g.head, r0);
+            for (int a = 0; a < C::kAtoms; ++a) ptx::tma_load_3d(dst + a * C::kAtomBytes, map, full, a * 64, head, r0);
           }
         }
         __syncwarp();
@@ -286,23 +328,29 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
       SegWalk walk(p);
       for (Segment g0; walk.next(p, g0);) {
         const Segment g = bcast_segment(g0);
-        if (g.n_tiles == 0) continue;
+        const SlotPlan sp = plan_of(p, g);
+        if (sp.n_it == 0) continue;
         ptx::mbar_wait(ptx::smem_u32(&bar.q_empty), (seg & 1) ^ 1);
         const uint32_t qf = ptx::smem_u32(&bar.q_full);
         if (ptx::elect_one()) {
-          ptx::mbar_arrive_expect_tx(qf, 2 * C::kTileBytes);
-#pragma unroll
-          for (int tile = 0; tile < 2; ++tile)
+          const int n_q = sp.single ? 1 : 2;  // a single unit keeps its one Q tile in Q slot 0 for both tile slots
+          ptx::mbar_arrive_expect_tx(qf, n_q * C::kTileBytes);
+          for (int tile = 0; tile < n_q; ++tile)
 #pragma unroll
             for (int a = 0; a < C::kAtoms; ++a)
               ptx::tma_load_3d(sQ + tile * C::kTileBytes + a * C::kAtomBytes, &p.map_q, qf, a * 64, g.head,
-                               g.pair * kPairM + tile * kBlockM);
+                               (sp.q_tile[0] + tile) * kBlockM);
         }
         __syncwarp();
-        load_kv(g, g.j0, false);
-        for (int j = g.j0; j < g.j1; ++j) {
-          load_kv(g, j, true);
-          if (j + 1 < g.j1) load_kv(g, j + 1, false);
+        load_kv(g.head, sp.jb[0], false);
+        if (sp.single) load_kv(g.head, sp.jb[1], false);
+        for (int k = 0; k < sp.n_it; ++k) {
+          load_kv(g.head, sp.jb[0] + k, true);
+          if (sp.single) load_kv(g.head, sp.jb[1] + k, true);
+          if (k + 1 < sp.n_it) {
+            load_kv(g.head, sp.jb[0] + k + 1, false);
+            if (sp.single) load_kv(g.head, sp.jb[1] + k + 1, false);
+          }
         }
         ++seg;
       }
@@ -315,9 +363,9 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
       constexpr uint64_t kDescV = ((uint64_t)(C::kAtomBytes >> 4) << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
       const uint64_t dQ = kDescK | (uint64_t)((sQ & 0x3FFFFu) >> 4);
       const uint64_t dKV = (uint64_t)((sKV & 0x3FFFFu) >> 4);
-      // S(tile) = Q(tile) . K(slot)^T
-      auto issue_qk = [&](int tile, uint32_t slot) {
-        const uint64_t qa = dQ + (uint64_t)(tile * (C::kTileBytes >> 4));
+      // S(tile) = Q(q_slot) . K(slot)^T
+      auto issue_qk = [&](int tile, int q_slot, uint32_t slot) {
+        const uint64_t qa = dQ + (uint64_t)(q_slot * (C::kTileBytes >> 4));
         const uint64_t kb = (kDescK | dKV) + (uint64_t)(slot * (C::kTileBytes >> 4));
         const uint32_t ts = tmem_u + (tile ? C::kTmemS1 : C::kTmemS0);
 #pragma unroll
@@ -326,7 +374,7 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
           ptx::mma_ss(ts, qa + off, kb + off, C::kIdescQK, k > 0);
         }
       };
-      // O(tile) (+)= P(tile)[:, 32*chunk .. 32*chunk+32) . V(slot)[32*chunk .. , :]
+      // O(tile) (+)= P(tile)[:, 16-key units of chunk] . V(slot)[those keys, :]
       auto issue_pv = [&](int tile, uint32_t slot, int chunk, bool acc) {
         const uint64_t vb = (kDescV | dKV) + (uint64_t)(slot * (C::kTileBytes >> 4));
         const uint32_t ts = tmem_u + (tile ? C::kTmemS1 : C::kTmemS0);
@@ -343,30 +391,40 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
       SegWalk walk(p);
       for (Segment g0; walk.next(p, g0);) {
         const Segment g = bcast_segment(g0);
-        if (g.n_tiles == 0) continue;
+        const SlotPlan sp = plan_of(p, g);
+        if (sp.n_it == 0) continue;
+        const bool split = sp.single;     // the slots use separate K/V tiles
+        const int q_slot1 = split ? 0 : 1;
         ptx::mbar_wait(ptx::smem_u32(&bar.q_full), seg & 1);
-        wait_full(it);
         {
-          const uint32_t slot = it % kStages;
+          const uint32_t it_a = it++, it_b = split ? it++ : it_a;
+          wait_full(it_a);
           if (ptx::elect_one()) {
-            issue_qk(0, slot);
+            issue_qk(0, 0, it_a % kStages);
             ptx::tc_commit(ptx::smem_u32(&bar.s_full[0]));
-            issue_qk(1, slot);
-            ptx::tc_commit(ptx::smem_u32(&bar.s_full[1]));
-            ptx::tc_commit(ptx::smem_u32(&bar.kv_empty[slot]));
-            if (g.j0 + 1 == g.j1) ptx::tc_commit(ptx::smem_u32(&bar.q_empty));
+            if (split) ptx::tc_commit(ptx::smem_u32(&bar.kv_empty[it_a % kStages]));
           }
           __syncwarp();
-          ++it;
+          if (split) wait_full(it_b);
+          if (ptx::elect_one()) {
+            issue_qk(1, q_slot1, it_b % kStages);
+            ptx::tc_commit(ptx::smem_u32(&bar.s_full[1]));
+            ptx::tc_commit(ptx::smem_u32(&bar.kv_empty[it_b % kStages]));
+            if (sp.n_it == 1) ptx::tc_commit(ptx::smem_u32(&bar.q_empty));
+          }
+          __syncwarp();
         }
-        for (int j = g.j0; j < g.j1; ++j) {
-          const bool has_next = j + 1 < g.j1, acc = j > g.j0;
-          const uint32_t it_v = it++, slot_v = it_v % kStages;
-          uint32_t it_k = 0, slot_k = 0;
-          if (has_next) { it_k = it++; slot_k = it_k % kStages; }
-          wait_full(it_v);
+        for (int k = 0; k < sp.n_it; ++k) {
+          const bool has_next = k + 1 < sp.n_it, acc = k > 0;
+          uint32_t it_v[2], it_k[2] = {0, 0};
+          it_v[0] = it++;
+          it_v[1] = split ? it++ : it_v[0];
+          if (has_next) { it_k[0] = it++; it_k[1] = split ? it++ : it_k[0]; }
+          wait_full(it_v[0]);
 #pragma unroll
           for (int tile = 0; tile < 2; ++tile) {
+            const uint32_t slot_v = it_v[tile] % kStages, slot_k = it_k[tile] % kStages;
+            if (tile == 1 && split) wait_full(it_v[1]);
 #pragma unroll
             for (int c = 0; c + 1 < kPChunks; ++c) {
               ptx::mbar_wait(ptx::smem_u32(&bar.p_ready[tile][c]), p_phase);
@@ -376,18 +434,16 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
             }
             ptx::mbar_wait(ptx::smem_u32(&bar.p_ready[tile][kPChunks - 1]), p_phase);
             ptx::tc_fence_after();
-            if (tile == 0 && has_next) wait_full(it_k);
+            if (has_next && (tile == 0 || split)) wait_full(it_k[tile]);
             if (ptx::elect_one()) {
               issue_pv(tile, slot_v, kPChunks - 1, acc);
               ptx::tc_commit(ptx::smem_u32(&bar.o_done[tile]));
-              if (tile == 1) ptx::tc_commit(ptx::smem_u32(&bar.kv_empty[slot_v]));
+              if (tile == 1 || split) ptx::tc_commit(ptx::smem_u32(&bar.kv_empty[slot_v]));
               if (has_next) {
-                issue_qk(tile, slot_k);
+                issue_qk(tile, tile ? q_slot1 : 0, slot_k);
                 ptx::tc_commit(ptx::smem_u32(&bar.s_full[tile]));
-                if (tile == 1) {
-                  ptx::tc_commit(ptx::smem_u32(&bar.kv_empty[slot_k]));
-                  if (j + 2 == g.j1) ptx::tc_commit(ptx::smem_u32(&bar.q_empty));
-                }
+                if (tile == 1 || split) ptx::tc_commit(ptx::smem_u32(&bar.kv_empty[slot_k]));
+                if (tile == 1 && k + 2 == sp.n_it) ptx::tc_commit(ptx::smem_u32(&bar.q_empty));
               }
             }
             __syncwarp();
@@ -400,7 +456,7 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
   } else {
     // ============================== softmax warpgroups ==============================
     ptx::setmaxnreg_inc<224>();
-    const int tile = (warp - 4) >> 2;                    // 0 or 1: which Q tile of the pair
+    const int tile = (warp - 4) >> 2;                    // 0 or 1: which tile slot of the CTA
     const int row_in_tile = ((warp & 3) << 5) | lane;    // == TMEM lane this thread may access
     const uint32_t lane_off = (uint32_t)((warp & 3) << 5) << 16;
     const uint32_t tS = tmem + (tile ? C::kTmemS1 : C::kTmemS0) + lane_off;
@@ -410,13 +466,45 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
     const uint32_t o_done = ptx::smem_u32(&bar.o_done[tile]);
     uint32_t n_iter = 0;  // S tiles consumed so far == PVs requested so far (drives every phase bit)
 
+    // final rows: O / l in the output dtype, LSE
+    auto store_row = [&](int head, int row, float inv, uint32_t t_src, auto&& transform) {
+#pragma unroll
+      for (int ch = 0; ch < D / 32; ++ch) {
+        uint32_t o[32];
+        ptx::tmem_ld32(t_src + ch * 32, o);
+        ptx::tc_wait_ld();
+        transform(ch, o);
+        if (row < p.Lq) {
+          if constexpr (OUT_F32) {
+            float4* dst = reinterpret_cast<float4*>(reinterpret_cast<float*>(p.out) + ((int64_t)row * p.out_pitch + (int64_t)head * D) + ch * 32);
+#pragma unroll
+            for (int c = 0; c < 8; ++c)
+              dst[c] = make_float4(__uint_as_float(o[4 * c]) * inv, __uint_as_float(o[4 * c + 1]) * inv,
+                                   __uint_as_float(o[4 * c + 2]) * inv, __uint_as_float(o[4 * c + 3]) * inv);
+          } else {
+            uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<__nv_bfloat16*>(p.out) + ((int64_t)row * p.out_pitch + (int64_t)head * D) + ch * 32);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+              uint4 v;
+              v.x = ptx::pack_bf16(__uint_as_float(o[8 * c]) * inv, __uint_as_float(o[8 * c + 1]) * inv);
+              v.y = ptx::pack_bf16(__uint_as_float(o[8 * c + 2]) * inv, __uint_as_float(o[8 * c + 3]) * inv);
+              v.z = ptx::pack_bf16(__uint_as_float(o[8 * c + 4]) * inv, __uint_as_float(o[8 * c + 5]) * inv);
+              v.w = ptx::pack_bf16(__uint_as_float(o[8 * c + 6]) * inv, __uint_as_float(o[8 * c + 7]) * inv);
+              dst[c] = v;
+            }
+          }
+        }
+      }
+    };
+
     SegWalk walk(p);
     for (Segment g; walk.next(p, g);) {
-      const int row = g.pair * kPairM + tile * kBlockM + row_in_tile;
+      const SlotPlan sp = plan_of(p, g);
+      const int row = (tile ? sp.q_tile[1] : sp.q_tile[0]) * kBlockM + row_in_tile;
       const bool row_valid = row < p.Lq;
-      if (g.n_tiles == 0) {
-        // no key is visible to this Q-tile pair (reading R11): output rows 0, LSE -inf
-        if (row_valid) {
+      if (sp.n_it == 0) {
+        // no key is visible to this unit (reading R11): output rows 0, LSE -inf (a single unit: slot 0 writes them)
+        if (row_valid && !(sp.single && tile == 1)) {
           if (p.lse != nullptr) p.lse[(int64_t)g.head * p.Lq + row] = -INFINITY;
           constexpr int kRowVecs = D * (OUT_F32 ? 4 : 2) / 16;
           uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<char*>(p.out) + ((int64_t)row * p.out_pitch + (int64_t)g.head * D) * (OUT_F32 ? 4 : 2));
@@ -430,9 +518,11 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
       const int nvis = p.kv_visible[block_of_row(p, min(row, p.Lq - 1))];
       const int vis_cache = (int)min((int64_t)nvis, p.cache_len);
       float m = -INFINITY, l = 0.f;  // running max in raw-score units, running sum
+      const int j_begin = tile ? sp.jb[1] : sp.jb[0];
 
-      for (int j = g.j0; j < g.j1; ++j, ++n_iter) {
-        int lim;  // columns [0, lim) of this tile are visible to this row
+      for (int k = 0; k < sp.n_it; ++k, ++n_iter) {
+        const int j = j_begin + k;
+        int lim;  // columns [0, lim) of this tile are visible to this row (<= 0: none; a run past the visible range)
         if (j < p.n_cache_tiles) lim = vis_cache - j * kBlockN;
         else lim = nvis - (int)p.cache_len - (j - p.n_cache_tiles) * kBlockN;
 
@@ -463,7 +553,7 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
         const float mx = fmaxf(fmaxf(fmaxf(mx8[0], mx8[1]), fmaxf(mx8[2], mx8[3])), fmaxf(fmaxf(mx8[4], mx8[5]), fmaxf(mx8[6], mx8[7])));
         const float m_new = fmaxf(m, mx);
         const bool grow = (m_new - m) * p.scale_log2 > kRescaleThreshold;  // false when both are -inf (NaN)
-        if (j == g.j0) {
+        if (k == 0) {
           m = m_new;  // O is overwritten by the first P.V of the segment: nothing to rescale
         } else if (__any_sync(0xffffffffu, grow)) {
           // lazy rescale of the accumulator in TMEM: needs the previous P.V to have landed
@@ -482,7 +572,7 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
           }
         }
         const float neg_ms = (m == -INFINITY) ? 0.f : -m * p.scale_log2;
-        // P = 2^(s*scale - m*scale) in kPChunks chunks of 32 keys; each chunk is handed to the MMA warp as soon
+        // P = 2^(s*scale - m*scale) in kPChunks chunks; each chunk is handed to the MMA warp as soon
         // as it sits in TMEM, so that P.V of the early chunks overlaps the exponentials of the later ones.
         // Tiles in which some row of this warp has masked keys take the all-MUFU variant: ex2(-inf) is
         // exactly 0 there, while the polynomial clamps to 2^-126 (an empty row must sum to l == 0, R11).
@@ -520,43 +610,48 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
       // ------------------------------ segment epilogue ------------------------------
       ptx::mbar_wait(o_done, (n_iter - 1) & 1);
       ptx::tc_fence_after();
-      const bool whole = (g.j0 == 0 && g.j1 == g.n_tiles);
-      if (whole) {
+      const float m_l2 = m == -INFINITY ? -INFINITY : m * p.scale_log2;  // running max in log2 units
+      if (sp.whole && !sp.single) {
         const float inv = l > 0.f ? 1.f / l : 0.f;
-        if (p.lse != nullptr && row_valid)
-          p.lse[(int64_t)g.head * p.Lq + row] = l > 0.f ? (ptx::lg2(l) + m * p.scale_log2) * kLn2 : -INFINITY;
+        if (p.lse != nullptr && row_valid) p.lse[(int64_t)g.head * p.Lq + row] = l > 0.f ? (ptx::lg2(l) + m_l2) * kLn2 : -INFINITY;
+        store_row(g.head, row, inv, tO, [](int, uint32_t (&)[32]) {});
+      } else if (sp.whole) {
+        // single unit, whole KV range in this CTA: slot 1 publishes (m, l) and keeps its accumulator in TMEM; slot 0's
+        // thread of the same row (same TMEM lane) merges the two halves and writes the final row.
+        if (tile == 1) {
+          merge_ml[row_in_tile] = make_float2(m_l2, l);
+          ptx::tc_fence_before();
+          ptx::named_bar_arrive(1, 2 * kBlockM);  // "slot 1's half is complete"
+          ptx::named_bar_sync(2, 2 * kBlockM);    // slot 0 has read O1: the next segment may overwrite it
+        } else {
+          ptx::named_bar_sync(1, 2 * kBlockM);
+          ptx::tc_fence_after();
+          const float2 other = merge_ml[row_in_tile];
+          const float M = fmaxf(m_l2, other.x);
+          const float w0 = M == -INFINITY ? 0.f : ptx::ex2(m_l2 - M), w1 = M == -INFINITY ? 0.f : ptx::ex2(other.x - M);
+          const float L = w0 * l + w1 * other.y;
+          const float inv = L > 0.f ? 1.f / L : 0.f;
+          if (p.lse != nullptr && row_valid) p.lse[(int64_t)g.head * p.Lq + row] = L > 0.f ? (ptx::lg2(L) + M) * kLn2 : -INFINITY;
+          const uint32_t tO1 = tmem + C::kTmemO1 + lane_off;
+          store_row(g.head, row, inv, tO, [&](int ch, uint32_t (&o)[32]) {
+            uint32_t o1[32];
+            ptx::tmem_ld32(tO1 + ch * 32, o1);
+            ptx::tc_wait_ld();
 #pragma unroll
-        for (int ch = 0; ch < D / 32; ++ch) {
-          uint32_t o[32];
-          ptx::tmem_ld32(tO + ch * 32, o);
-          ptx::tc_wait_ld();
-          if (row_valid) {
-            if constexpr (OUT_F32) {
-              float4* dst = reinterpret_cast<float4*>(reinterpret_cast<float*>(p.out) + ((int64_t)row * p.out_pitch + (int64_t)g.head * D) + ch * 32);
-#pragma unroll
-              for (int c = 0; c < 8; ++c)
-                dst[c] = make_float4(__uint_as_float(o[4 * c]) * inv, __uint_as_float(o[4 * c + 1]) * inv,
-                                     __uint_as_float(o[4 * c + 2]) * inv, __uint_as_float(o[4 * c + 3]) * inv);
-            } else {
-              uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<__nv_bfloat16*>(p.out) + ((int64_t)row * p.out_pitch + (int64_t)g.head * D) + ch * 32);
-#pragma unroll
-              for (int c = 0; c < 4; ++c) {
-                uint4 v;
-                v.x = ptx::pack_bf16(__uint_as_float(o[8 * c]) * inv, __uint_as_float(o[8 * c + 1]) * inv);
-                v.y = ptx::pack_bf16(__uint_as_float(o[8 * c + 2]) * inv, __uint_as_float(o[8 * c + 3]) * inv);
-                v.z = ptx::pack_bf16(__uint_as_float(o[8 * c + 4]) * inv, __uint_as_float(o[8 * c + 5]) * inv);
-                v.w = ptx::pack_bf16(__uint_as_float(o[8 * c + 6]) * inv, __uint_as_float(o[8 * c + 7]) * inv);
-                dst[c] = v;
-              }
+            for (int c = 0; c < 32; ++c) {
+              // a half that saw no key (w == 0) may hold an accumulator that was never written: keep it out
+              const float a0 = w0 > 0.f ? w0 * __uint_as_float(o[c]) : 0.f, a1 = w1 > 0.f ? w1 * __uint_as_float(o1[c]) : 0.f;
+              o[c] = __float_as_uint(a0 + a1);
             }
-          }
+          });
+          ptx::tc_fence_before();
+          ptx::named_bar_arrive(2, 2 * kBlockM);
         }
       } else {
-        // partial: unnormalised O (FP32), running max (log2 units) and sum, into slot work + cta
-        const int64_t slot = (int64_t)g.head * p.n_pairs + g.pair + blockIdx.x;
-        const int r = tile * kBlockM + row_in_tile;
-        p.part_ml[slot * kPairM + r] = make_float2(m == -INFINITY ? -INFINITY : m * p.scale_log2, l);
-        float4* po = reinterpret_cast<float4*>(p.part_o) + slot * (D / 4) * kPairM + r;
+        // partial: unnormalised O (FP32), running max (log2 units) and sum, into record (item + cta) * 2 + slot
+        const int64_t rec = ((int64_t)g.head * p.n_units + g.unit + blockIdx.x) * 2 + tile;
+        p.part_ml[rec * kBlockM + row_in_tile] = make_float2(m_l2, l);
+        float4* po = reinterpret_cast<float4*>(p.part_o) + rec * (D / 4) * kBlockM + row_in_tile;
 #pragma unroll
         for (int ch = 0; ch < D / 32; ++ch) {
           uint32_t o[32];
@@ -564,11 +659,11 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
           ptx::tc_wait_ld();
 #pragma unroll
           for (int c = 0; c < 8; ++c)
-            po[(int64_t)(ch * 8 + c) * kPairM] = make_float4(__uint_as_float(o[4 * c]), __uint_as_float(o[4 * c + 1]),
-                                                             __uint_as_float(o[4 * c + 2]), __uint_as_float(o[4 * c + 3]));
+            po[(int64_t)(ch * 8 + c) * kBlockM] = make_float4(__uint_as_float(o[4 * c]), __uint_as_float(o[4 * c + 1]),
+                                                              __uint_as_float(o[4 * c + 2]), __uint_as_float(o[4 * c + 3]));
         }
       }
-      // the next segment's first P.V overwrites O: order our TMEM reads before the p_full arrive that unleashes it
+      // the next segment's first P.V overwrites O: order our TMEM reads before the p_ready arrive that unleashes it
       ptx::tc_fence_before();
     }
   }
@@ -579,36 +674,43 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
 }
 
 // ---------------------------------------------------------------------------------------------
-// combine kernel: merges the split-KV partials of the phase-2 items, and zero-fills phase-2 items
-// that see no key at all.  grid = (number of phase-2 items, d/4), block = 256 threads (one per row).
+// combine kernel: merges the split-KV partials of the phase-2 units, and zero-fills phase-2 units
+// that see no key at all.  grid = (number of phase-2 units, d/4), block = 256 threads: thread r handles
+// row r % 128 of tile slot r / 128 (a single unit has one Q tile: its slot-1 threads have nothing to do).
 // ---------------------------------------------------------------------------------------------
 template <int D, bool OUT_F32>
 __global__ void __launch_bounds__(kPairM) attn_combine_kernel(const __grid_constant__ Params p) {
   wsi::pdl_trigger();
   wsi::pdl_wait();  // the partials are the attention kernel's
-  const int w = p.n_waves * p.grid + blockIdx.x, head = w / p.n_pairs, pair = w - head * p.n_pairs;
-  const int q4 = blockIdx.y, r = threadIdx.x;
-  const int row = pair * kPairM + r;
+  const int w = p.n_waves * p.grid + blockIdx.x, head = w / p.n_units, unit = w - head * p.n_units;
+  const int q4 = blockIdx.y, slot = threadIdx.x >> 7, r = threadIdx.x & (kBlockM - 1);
+  const bool single = p.last_single && unit == p.n_units - 1;
+  if (single && slot == 1) return;
+  const int row = (2 * unit + slot) * kBlockM + r;
   if (row >= p.Lq) return;
-  const int Tp = p.pair_prefix[p.n_pairs];
-  const int n_tiles = p.pair_prefix[pair + 1] - p.pair_prefix[pair];
+  const int Tp = p.unit_prefix[p.n_units];
+  const int n_iters = p.unit_prefix[unit + 1] - p.unit_prefix[unit];
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
   float lse = -INFINITY;
-  if (n_tiles > 0) {
-    const int64_t a = (int64_t)head * Tp + p.pair_prefix[pair];
-    const int c_lo = cta_of_iter(p, a), c_hi = cta_of_iter(p, a + n_tiles - 1);
+  if (n_iters > 0) {
+    const int64_t a = (int64_t)head * Tp + p.unit_prefix[unit];
+    const int c_lo = cta_of_iter(p, a), c_hi = cta_of_iter(p, a + n_iters - 1);
     if (c_lo == c_hi) return;  // one CTA covered the whole KV range and wrote the final rows itself
+    // records (w + c) * 2 + s: a pair's tile slot s has one record per CTA (stride 2); a single unit's tile has both
+    // slots' records of every CTA (stride 1)
+    const int64_t rec0 = ((int64_t)w + c_lo) * 2 + (single ? 0 : slot);
+    const int n_rec = (c_hi - c_lo + 1) * (single ? 2 : 1), stride = single ? 1 : 2;
     // online LSE-weighted merge, four partials per step so that eight independent loads are in flight per thread
     float M = -INFINITY, L = 0.f;
-    for (int c = c_lo; c <= c_hi; c += 4) {
+    for (int k = 0; k < n_rec; k += 4) {
       float2 ml[4];
       float4 o[4];
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
-        const int64_t slot = (int64_t)w + min(c + u, c_hi);
-        ml[u] = p.part_ml[slot * kPairM + r];
-        o[u] = reinterpret_cast<const float4*>(p.part_o)[(slot * (D / 4) + q4) * kPairM + r];
-        if (c + u > c_hi) ml[u] = make_float2(-INFINITY, 0.f);
+        const int64_t rec = rec0 + (int64_t)min(k + u, n_rec - 1) * stride;
+        ml[u] = p.part_ml[rec * kBlockM + r];
+        o[u] = reinterpret_cast<const float4*>(p.part_o)[(rec * (D / 4) + q4) * kBlockM + r];
+        if (k + u >= n_rec) ml[u] = make_float2(-INFINITY, 0.f);
       }
       const float M_new = fmaxf(fmaxf(M, fmaxf(ml[0].x, ml[1].x)), fmaxf(ml[2].x, ml[3].x));
       if (M_new > -INFINITY) {
@@ -617,7 +719,8 @@ __global__ void __launch_bounds__(kPairM) attn_combine_kernel(const __grid_const
         L *= f;
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
-          const float wgt = ptx::ex2(ml[u].x - M_new);  // 0 for an all-masked partial (m = -inf)
+          if (ml[u].x == -INFINITY) continue;  // a partial that saw no key: weight 0, accumulator not meaningful
+          const float wgt = ptx::ex2(ml[u].x - M_new);
           acc.x += wgt * o[u].x; acc.y += wgt * o[u].y; acc.z += wgt * o[u].z; acc.w += wgt * o[u].w;
           L += wgt * ml[u].y;
         }
@@ -737,8 +840,8 @@ struct WsLayout {
 WsLayout ws_layout(int32_t Lq, int32_t H, int32_t d, int64_t kv_total, int64_t cache_len, int32_t Ln, ws_dtype dt,
                    bool exact) {
   WsLayout L{};
-  const size_t n_pairs = (size_t)(Lq + kPairM - 1) / kPairM;
-  const size_t slots = n_pairs * H + kMaxCtas;
+  const size_t n_units = (size_t)(Lq + kPairM - 1) / kPairM;
+  const size_t slots = n_units * H + kMaxCtas;  // x 2 records of 128 rows each
   size_t off = 0;
   L.part_o = off; off = align_up(off + slots * kPairM * (size_t)d * 4, 256);
   L.part_ml = off; off = align_up(off + slots * kPairM * 8, 256);
@@ -768,9 +871,9 @@ int launch_attention(const Params& prm, DeviceState* st, cudaStream_t stream) {
     if (e != cudaSuccess) return wsi::cuda_fail(e);
     ++launches;
   }
-  const int n_pool_items = prm.H * prm.n_pairs - prm.n_waves * prm.grid;
+  const int n_pool_items = prm.H * prm.n_units - prm.n_waves * prm.grid;
   if (n_pool_items > 0) {
-    dim3 cgrid((unsigned)n_pool_items, D / 4);  // items on x: H * n_pairs may exceed the 65535 limit of y
+    dim3 cgrid((unsigned)n_pool_items, D / 4);  // items on x: H * n_units may exceed the 65535 limit of y
     const cudaError_t e = wsi::launch_pdl(attn_combine_kernel<D, OUT_F32>, cgrid, dim3(kPairM), 0, stream, prm);
     if (e != cudaSuccess) return wsi::cuda_fail(e);
     ++launches;
@@ -786,34 +889,49 @@ extern "C" __attribute__((visibility("default"))) size_t ws_block_causal_attn_wo
 }
 
 namespace {
-// KV-tile iterations of every Q-tile pair: a pair visits the KV tiles its last row can see.  Fills
-// prm.pair_prefix / n_cache_tiles (needs prm.n_pairs) and returns the iterations per head.
-int64_t build_pair_prefix(Params& prm, const ws_block_mask* mask, int32_t Lq, int64_t cache_len) {
+// KV tiles the last row of Q tile `qt` can see (a tile visits exactly those).
+int64_t kv_tiles_of_q_tile(const ws_block_mask* mask, int32_t Lq, int64_t cache_len, int qt) {
+  const int last_row = ((qt + 1) * kBlockM < Lq ? (qt + 1) * kBlockM : Lq) - 1;
+  int b = 0;
+  while (last_row >= mask->q_block_end[b]) ++b;
+  const int64_t nvis = mask->kv_visible[b];
+  if (nvis <= 0) return 0;
+  const int64_t nct = (cache_len + kBlockN - 1) / kBlockN;
+  return nvis <= cache_len ? (nvis + kBlockN - 1) / kBlockN : nct + (nvis - cache_len + kBlockN - 1) / kBlockN;
+}
+
+// Work units of a head and their iteration counts: Q tiles (2u, 2u + 1) form pair unit u, which runs one iteration
+// per KV tile its later tile sees; an odd last Q tile is a single unit, whose KV tiles are cut in two runs (one per
+// tile slot), i.e. one iteration per two KV tiles.  Fills prm.unit_prefix / n_cache_tiles / last_* (needs
+// prm.n_units) and returns the iterations per head.  unit_kv_tiles (optional): KV tiles each unit visits.
+int64_t build_unit_prefix(Params& prm, const ws_block_mask* mask, int32_t Lq, int64_t cache_len, int32_t* unit_kv_tiles) {
   prm.n_cache_tiles = (int)((cache_len + kBlockN - 1) / kBlockN);
+  const int n_q_tiles = (Lq + kBlockM - 1) / kBlockM;
+  prm.last_single = n_q_tiles & 1;
+  prm.last_kv_tiles = 0;
   int64_t Tp = 0;
-  prm.pair_prefix[0] = 0;
-  for (int pr = 0; pr < prm.n_pairs; ++pr) {
-    const int last_row = ((pr + 1) * kPairM < Lq ? (pr + 1) * kPairM : Lq) - 1;
-    int b = 0;
-    while (last_row >= mask->q_block_end[b]) ++b;
-    const int64_t nvis = mask->kv_visible[b];
-    if (nvis > 0)
-      Tp += nvis <= cache_len ? (nvis + kBlockN - 1) / kBlockN : prm.n_cache_tiles + (nvis - cache_len + kBlockN - 1) / kBlockN;
-    prm.pair_prefix[pr + 1] = (int32_t)Tp;
+  prm.unit_prefix[0] = 0;
+  for (int u = 0; u < prm.n_units; ++u) {
+    const bool single = prm.last_single && u == prm.n_units - 1;
+    const int64_t n = kv_tiles_of_q_tile(mask, Lq, cache_len, single ? 2 * u : 2 * u + 1);
+    if (single) prm.last_kv_tiles = (int32_t)n;
+    if (unit_kv_tiles) unit_kv_tiles[u] = (int32_t)n;
+    Tp += single ? (n + 1) / 2 : n;
+    prm.unit_prefix[u + 1] = (int32_t)Tp;
   }
   return Tp;
 }
 
 // The two-phase schedule (see Params) for a device with `sms` SMs: fills prm.grid, n_waves, pool_begin.
 void build_schedule(Params& prm, int64_t Tp, int sms) {
-  const int n_pairs = prm.n_pairs, H = prm.H;
-  const int64_t T = Tp * H, n_items = (int64_t)H * n_pairs;
+  const int n_units = prm.n_units, H = prm.H;
+  const int64_t T = Tp * H, n_items = (int64_t)H * n_units;
   int64_t G = T > 0 ? T : n_items;
   if (G > sms) G = sms;
   if (G > kMaxCtas) G = kMaxCtas;
   prm.grid = (int32_t)G;
-  auto item_len = [&](int64_t i) { const int pr = (int)(i % n_pairs); return (int64_t)(prm.pair_prefix[pr + 1] - prm.pair_prefix[pr]); };
-  auto item_flat = [&](int64_t i) { return (i / n_pairs) * Tp + prm.pair_prefix[i % n_pairs]; };
+  auto item_len = [&](int64_t i) { const int u = (int)(i % n_units); return (int64_t)(prm.unit_prefix[u + 1] - prm.unit_prefix[u]); };
+  auto item_flat = [&](int64_t i) { return (i / n_units) * Tp + prm.unit_prefix[i % n_units]; };
   // candidate B: W whole-item waves, the remaining items water-filled over the CTAs
   const int64_t W = n_items / G;
   int64_t p1[kMaxCtas], quota[kMaxCtas];
@@ -837,7 +955,7 @@ void build_schedule(Params& prm, int64_t Tp, int sms) {
   for (int64_t c = G - 1; c >= 0 && excess > 0; --c)
     if (quota[c] > 0) { --quota[c]; --excess; }
   const int64_t makespan_b = lo > p1_max ? lo : p1_max, makespan_a = (T + G - 1) / G;
-  // B trades a slightly longer critical path for far fewer split items and L2 reuse of K/V across the pairs of a head
+  // B trades a slightly longer critical path for far fewer split items and L2 reuse of K/V across the units of a head
   const bool use_b = W > 0 && makespan_b * 100 <= makespan_a * 103;
   if (use_b) {
     prm.n_waves = (int32_t)W;
@@ -867,20 +985,21 @@ int check_mask(const ws_block_mask* mask, int32_t Lq, int64_t cache_len, int32_t
 
 // Host-only diagnostic: the schedule ws_block_causal_attn uses for this problem on a device with n_sms SMs.
 extern "C" __attribute__((visibility("default"))) int ws_attn_schedule(int32_t Lq, int32_t H, int64_t cache_len, int32_t Ln, const ws_block_mask* mask,
-                                int32_t n_sms, int32_t* grid, int32_t* n_waves, int32_t* pair_tiles, int64_t* pool_begin) {
-  if (Lq <= 0 || H <= 0 || cache_len < 0 || Ln < 0 || n_sms <= 0 || !grid || !n_waves || !pair_tiles || !pool_begin)
+                                int32_t n_sms, int32_t* grid, int32_t* n_waves, int32_t* unit_iters, int32_t* unit_kv_tiles,
+                                int64_t* pool_begin) {
+  if (Lq <= 0 || H <= 0 || cache_len < 0 || Ln < 0 || n_sms <= 0 || !grid || !n_waves || !unit_iters || !unit_kv_tiles || !pool_begin)
     return WS_ERR_INVALID_ARG;
   if (const int rc = check_mask(mask, Lq, cache_len, Ln)) return rc;
-  if (cache_len + Ln > 0x7fffffffLL / kMaxPairs - kBlockN) return WS_ERR_UNSUPPORTED;
+  if (cache_len + Ln > 0x7fffffffLL / kMaxUnits - kBlockN) return WS_ERR_UNSUPPORTED;
   Params* prm = new Params();
   prm->Lq = Lq; prm->H = H; prm->Ln = Ln; prm->cache_len = cache_len;
-  prm->n_pairs = (Lq + kPairM - 1) / kPairM;
-  if (prm->n_pairs > kMaxPairs) { delete prm; return WS_ERR_UNSUPPORTED; }
-  const int64_t Tp = build_pair_prefix(*prm, mask, Lq, cache_len);
+  prm->n_units = (Lq + kPairM - 1) / kPairM;
+  if (prm->n_units > kMaxUnits) { delete prm; return WS_ERR_UNSUPPORTED; }
+  const int64_t Tp = build_unit_prefix(*prm, mask, Lq, cache_len, unit_kv_tiles);
   build_schedule(*prm, Tp, n_sms);
   *grid = prm->grid;
   *n_waves = prm->n_waves;
-  for (int pr = 0; pr < prm->n_pairs; ++pr) pair_tiles[pr] = prm->pair_prefix[pr + 1] - prm->pair_prefix[pr];
+  for (int u = 0; u < prm->n_units; ++u) unit_iters[u] = prm->unit_prefix[u + 1] - prm->unit_prefix[u];
   for (int c = 0; c <= prm->grid; ++c) pool_begin[c] = prm->pool_begin[c];
   delete prm;
   return WS_OK;
@@ -898,9 +1017,9 @@ int wsi::attn_validate(const void* out, const float* lse, const void* q, const v
   if ((Ln > 0) != (k_new != nullptr) || (Ln > 0) != (v_new != nullptr)) return WS_ERR_INVALID_ARG;
   if (cache_len > capacity) return WS_ERR_OUT_OF_RANGE;
   if (cache_len > 0 && (!k_cache || !v_cache)) return WS_ERR_INVALID_ARG;
-  if (cache_len + Ln > 0x7fffffffLL / kMaxPairs - kBlockN) return WS_ERR_UNSUPPORTED;  // pair_prefix is int32
+  if (cache_len + Ln > 0x7fffffffLL / kMaxUnits - kBlockN) return WS_ERR_UNSUPPORTED;  // unit_prefix is int32
   if (const int rc = check_mask(mask, Lq, cache_len, Ln)) return rc;
-  if ((Lq + kPairM - 1) / kPairM > kMaxPairs) return WS_ERR_UNSUPPORTED;
+  if ((Lq + kPairM - 1) / kPairM > kMaxUnits) return WS_ERR_UNSUPPORTED;
   if (!wsi::aligned16(out) || !wsi::aligned16(q) || !wsi::aligned16(k_cache) || !wsi::aligned16(v_cache) ||
       !wsi::aligned16(k_new) || !wsi::aligned16(v_new) || (lse && (reinterpret_cast<uintptr_t>(lse) & 3)))
     return WS_ERR_ALIGNMENT;
@@ -922,7 +1041,7 @@ int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const v
   if (const int rc = wsi::attn_validate(out, lse, q, k_cache, v_cache, capacity, cache_len, k_new, v_new, Ln, H, d, Lq, mask,
                                         softmax_scale, workspace, workspace_bytes, dt))
     return rc;
-  const int n_pairs = (Lq + kPairM - 1) / kPairM;
+  const int n_units = (Lq + kPairM - 1) / kPairM;
   const WsLayout L = ws_layout(Lq, H, d, cache_len + Ln, cache_len, Ln, dt, true);
   if (!get_encode_fn()) return wsi::cuda_fail(cudaErrorNotSupported);
   cudaError_t dev_err = cudaErrorNoDevice;
@@ -960,7 +1079,7 @@ int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const v
   prm.part_o = reinterpret_cast<float*>(ws + L.part_o);
   prm.part_ml = reinterpret_cast<float2*>(ws + L.part_ml);
   prm.cache_len = cache_len;
-  prm.Lq = Lq; prm.H = H; prm.Ln = Ln; prm.n_blocks = mask->n_blocks; prm.n_pairs = n_pairs;
+  prm.Lq = Lq; prm.H = H; prm.Ln = Ln; prm.n_blocks = mask->n_blocks; prm.n_units = n_units;
   prm.n_cache_tiles = (int)((cache_len + kBlockN - 1) / kBlockN);
   prm.scale = softmax_scale;
   // clamped away from 0 so that a masked (-inf) logit times the scale stays -inf (softmax_scale == 0 is legal)
@@ -969,7 +1088,7 @@ int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const v
     prm.q_block_end[b] = mask->q_block_end[b];
     prm.kv_visible[b] = mask->kv_visible[b];
   }
-  const int64_t Tp = build_pair_prefix(prm, mask, Lq, cache_len);
+  const int64_t Tp = build_unit_prefix(prm, mask, Lq, cache_len, nullptr);
   build_schedule(prm, Tp, dev->sms);
 
   // ---- launches ----

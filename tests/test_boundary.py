@@ -161,12 +161,12 @@ def test_attention_accepts_more_than_65535_work_items(lib):
     already run; the item index now sits on gridDim.x.  The schedule for such a problem must build."""
     n_sms = 148
     grid, n_waves = ctypes.c_int32(), ctypes.c_int32()
-    tiles = (ctypes.c_int32 * 4)()
+    iters, tiles = (ctypes.c_int32 * 4)(), (ctypes.c_int32 * 4)()
     pool = (ctypes.c_int64 * (n_sms + 1))()
     Mask = binding._BlockMask
     m = Mask(1, (ctypes.c_int32 * 1)(520), (ctypes.c_int32 * 1)(300))
-    H = 40000  # x 3 pairs = 120000 items
-    assert lib.ws_attn_schedule(520, H, 300, 0, ctypes.byref(m), n_sms, ctypes.byref(grid), ctypes.byref(n_waves), tiles, pool) == OK
+    H = 40000  # x 3 units = 120000 items
+    assert lib.ws_attn_schedule(520, H, 300, 0, ctypes.byref(m), n_sms, ctypes.byref(grid), ctypes.byref(n_waves), iters, tiles, pool) == OK
     assert grid.value == n_sms and n_waves.value == (H * 3) // n_sms
 
 

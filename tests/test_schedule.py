@@ -1,6 +1,6 @@
-"""Host logic of the attention work schedule (ws_attn_schedule), no GPU needed: every KV-tile
-iteration of every (head, Q-pair) work item is assigned to exactly one CTA, the loads are balanced, and the
-BASELINE.json configs take the schedules DESIGN.md says they take."""
+"""Host logic of the attention work schedule (ws_attn_schedule), no GPU needed: every (head, Q tile,
+KV tile) step is assigned to exactly one CTA tile slot, the loads are balanced, and the BASELINE.json configs take the
+schedules DESIGN.md says they take."""
 import math
 
 import pytest
@@ -9,23 +9,39 @@ import paper_2607_04443_b200 as ws
 from paper_2607_04443_b200 import workloads as wl
 
 
-def expand(plan, H):
-    """-> per-CTA list of (item, tile) and per-CTA load."""
-    tiles, grid, waves, pool = plan["pair_tiles"], plan["grid"], plan["n_waves"], plan["pool_begin"]
-    n_pairs, Tp = len(tiles), sum(tiles)
+def expand(plan, H, n_q_tiles):
+    """-> per-CTA list of (head, q_tile, kv_tile) steps, and per-CTA iteration counts.  Mirrors the documented
+    meaning of the schedule (ws.h): pair units run both Q tiles on every KV tile of the unit; iterations [i0, i1) of
+    a single unit cover its KV tiles [2 i0, min(2 i1, n))."""
+    iters, tiles, grid, waves, pool = plan["unit_iters"], plan["unit_kv_tiles"], plan["grid"], plan["n_waves"], plan["pool_begin"]
+    n_units, Tp = len(iters), sum(iters)
     prefix = [0]
-    for t in tiles:
+    for t in iters:
         prefix.append(prefix[-1] + t)
-    work = [[] for _ in range(grid)]
+    single_last = n_q_tiles % 2 == 1
+    steps = [[] for _ in range(grid)]
+    load = [0] * grid
+
+    def segment(c, head, u, i0, i1):
+        load[c] += i1 - i0
+        if single_last and u == n_units - 1:
+            steps[c] += [(head, 2 * u, j) for j in range(2 * i0, min(2 * i1, tiles[u]))]
+        else:
+            steps[c] += [(head, 2 * u + s, j) for j in range(i0, i1) for s in (0, 1)]
+
     for c in range(grid):
         for w in range(waves):
             item = w * grid + c
-            work[c] += [(item, j) for j in range(tiles[item % n_pairs])]
-        for t in range(pool[c], pool[c + 1]):
+            segment(c, item // n_units, item % n_units, 0, iters[item % n_units])
+        t = pool[c]
+        while t < pool[c + 1]:
             head, rem = divmod(t, Tp)
-            pair = max(p for p in range(n_pairs) if prefix[p] <= rem and tiles[p] > 0 and rem < prefix[p + 1])
-            work[c].append((head * n_pairs + pair, rem - prefix[pair]))
-    return work
+            u = max(k for k in range(n_units) if prefix[k] <= rem and iters[k] > 0 and rem < prefix[k + 1])
+            i0 = rem - prefix[u]
+            i1 = min(iters[u], i0 + pool[c + 1] - t)
+            segment(c, head, u, i0, i1)
+            t += i1 - i0
+    return steps, load
 
 
 def tiles_of(kv_vis, cache_len):
@@ -50,34 +66,48 @@ CASES = [
 ]
 
 
+CASES += [
+    (292, 24, 8192, 292, [292], [8484], 148),                                      # three Q tiles: a pair and a single
+    (128, 8, 4000, 0, [128], [4000], 148),                                         # one Q tile per head: singles only
+    (100, 3, 0, 100, [100], [100], 148),                                           # a single with ONE KV tile
+    (3 * 128, 5, 1000, 384, [128, 256, 384], [1128, 1256, 1384], 148),             # the single tile sees the most
+    (300, 4, 200, 44, [256, 300], [100, 244], 16),                                 # the single tile sees more than the pair
+]
+
+
 @pytest.mark.parametrize("case", CASES)
-def test_every_iteration_is_assigned_exactly_once_and_loads_are_balanced(case):
+def test_every_step_is_assigned_exactly_once_and_loads_are_balanced(case):
     Lq, H, Tc, Ln, qe, kv, sms = case
     plan = ws.attn_schedule(Lq, H, Tc, Ln, qe, kv, sms)
-    n_pairs = math.ceil(Lq / 256)
-    # tiles per pair follow the last row of the pair
-    want = []
-    for p in range(n_pairs):
-        last = min((p + 1) * 256, Lq) - 1
+    n_q_tiles, n_units = math.ceil(Lq / 128), math.ceil(Lq / 256)
+
+    def kv_tiles_of_q_tile(qt):  # a Q tile visits the KV tiles its last row sees
+        last = min((qt + 1) * 128, Lq) - 1
         b = next(i for i, e in enumerate(qe) if last < e)
-        want.append(tiles_of(kv[b], Tc))
-    assert plan["pair_tiles"] == want
-    T = sum(want) * H
+        return tiles_of(kv[b], Tc)
+
+    want_tiles, want_iters = [], []
+    for u in range(n_units):
+        single = n_q_tiles % 2 == 1 and u == n_units - 1
+        n = kv_tiles_of_q_tile(2 * u if single else 2 * u + 1)
+        want_tiles.append(n)
+        want_iters.append((n + 1) // 2 if single else n)
+    assert plan["unit_kv_tiles"] == want_tiles and plan["unit_iters"] == want_iters
+    T = sum(want_iters) * H
     assert 1 <= plan["grid"] <= sms
     assert plan["pool_begin"] == sorted(plan["pool_begin"])
-    work = expand(plan, H)
-    flat = [x for w in work for x in w]
-    assert len(flat) == T and len(set(flat)) == T, "some iteration is missing or assigned twice"
-    assert set(flat) == {(h * n_pairs + p, j) for h in range(H) for p in range(n_pairs) for j in range(want[p])}
-    # phase-1 items are whole and phase-2 items are the tail of the item order
-    first_pool_item = plan["n_waves"] * plan["grid"]
-    for c, w in enumerate(work):
-        for item, _ in w[sum(want[(k * plan["grid"] + c) % n_pairs] for k in range(plan["n_waves"])):]:
-            assert item >= first_pool_item
+    steps, load = expand(plan, H, n_q_tiles)
+    flat = [x for w in steps for x in w]
+    assert len(set(flat)) == len(flat), "some step is assigned twice"
+    # every KV tile a Q tile can see is covered (a pair's earlier tile may additionally run tiles it cannot see: masked)
+    need = {(h, qt, j) for h in range(H) for qt in range(n_q_tiles) for j in range(kv_tiles_of_q_tile(qt))}
+    assert need <= set(flat), "some visible (head, Q tile, KV tile) step is missing"
+    extra = set(flat) - need
+    assert all(qt % 2 == 0 and qt + 1 < n_q_tiles for _, qt, _ in extra), "only a pair's earlier tile may run invisible tiles"
+    assert sum(load) == T
     # balance: within 3 % (+1 iteration) of the perfectly even split
     if T:
-        loads = [len(w) for w in work]
-        assert max(loads) <= math.ceil(T / plan["grid"]) * 1.03 + 1
+        assert max(load) <= math.ceil(T / plan["grid"]) * 1.03 + 1
 
 
 def test_baseline_configs_take_the_documented_schedules():
@@ -85,11 +115,13 @@ def test_baseline_configs_take_the_documented_schedules():
         c = wl.CONFIGS[name]
         return ws.attn_schedule(c.Lq, c.H, c.cache_len, c.Ln, list(c.q_block_end), list(c.kv_visible), 148)
     p3, p4, p2, p5 = plan("cfg3"), plan("cfg4"), plan("cfg2"), plan("cfg5")
-    assert (p3["grid"], p3["n_waves"], p3["pair_tiles"]) == (148, 1, [136] * 4)       # 148 whole items + 12 split ones
+    assert (p3["grid"], p3["n_waves"], p3["unit_iters"]) == (148, 1, [136] * 4)       # 148 whole items + 12 split ones
     assert p3["pool_begin"][0] == 37 * 4 * 136 and p3["pool_begin"][-1] == 160 * 136
     assert (p5["grid"], p5["n_waves"]) == (148, 1)
-    assert p4["n_waves"] == 0 and p4["pool_begin"][-1] == 10 * sum(p4["pair_tiles"])   # unequal items: pure stream-K
-    assert p2["n_waves"] == 0 and p2["pair_tiles"] == [67, 67]                         # fewer items than SMs
+    assert p4["n_waves"] == 0 and p4["pool_begin"][-1] == 10 * sum(p4["unit_iters"])   # unequal items: pure stream-K
+    assert len(p4["unit_iters"]) == 15 and p4["unit_iters"][-1] == (p4["unit_kv_tiles"][-1] + 1) // 2  # 29 Q tiles: 14 pairs + a single
+    # cfg2: 292 rows = a pair (67 KV tiles) and a single tile that walks its 67 KV tiles two per iteration
+    assert p2["n_waves"] == 0 and p2["unit_iters"] == [67, 34] and p2["unit_kv_tiles"] == [67, 67]
 
 
 def test_schedule_rejects_bad_masks():
