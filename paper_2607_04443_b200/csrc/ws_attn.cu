@@ -650,17 +650,19 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
       } else {
         // partial: unnormalised O (FP32), running max (log2 units) and sum, into record (item + cta) * 2 + slot
         const int64_t rec = ((int64_t)g.head * p.n_units + g.unit + blockIdx.x) * 2 + tile;
-        p.part_ml[rec * kBlockM + row_in_tile] = make_float2(m_l2, l);
+        if (row_valid) p.part_ml[rec * kBlockM + row_in_tile] = make_float2(m_l2, l);
         float4* po = reinterpret_cast<float4*>(p.part_o) + rec * (D / 4) * kBlockM + row_in_tile;
 #pragma unroll
         for (int ch = 0; ch < D / 32; ++ch) {
           uint32_t o[32];
           ptx::tmem_ld32(tO + ch * 32, o);
           ptx::tc_wait_ld();
+          if (row_valid) {  // padding rows are never read by the combine kernel
 #pragma unroll
-          for (int c = 0; c < 8; ++c)
-            po[(int64_t)(ch * 8 + c) * kBlockM] = make_float4(__uint_as_float(o[4 * c]), __uint_as_float(o[4 * c + 1]),
-                                                              __uint_as_float(o[4 * c + 2]), __uint_as_float(o[4 * c + 3]));
+            for (int c = 0; c < 8; ++c)
+              po[(int64_t)(ch * 8 + c) * kBlockM] = make_float4(__uint_as_float(o[4 * c]), __uint_as_float(o[4 * c + 1]),
+                                                                __uint_as_float(o[4 * c + 2]), __uint_as_float(o[4 * c + 3]));
+          }
         }
       }
       // the next segment's first P.V overwrites O: order our TMEM reads before the p_ready arrive that unleashes it
@@ -700,25 +702,32 @@ __global__ void __launch_bounds__(kPairM) attn_combine_kernel(const __grid_const
     // slots' records of every CTA (stride 1)
     const int64_t rec0 = ((int64_t)w + c_lo) * 2 + (single ? 0 : slot);
     const int n_rec = (c_hi - c_lo + 1) * (single ? 2 : 1), stride = single ? 1 : 2;
-    // online LSE-weighted merge, four partials per step so that eight independent loads are in flight per thread
+    // online LSE-weighted merge, four partials per step with all eight loads of a step in flight at once (the kernel
+    // is a chain of dependent L2 round trips otherwise; eight partials per step cost occupancy and measured slower)
+    constexpr int kBatch = 4;
     float M = -INFINITY, L = 0.f;
-    for (int k = 0; k < n_rec; k += 4) {
-      float2 ml[4];
-      float4 o[4];
+    for (int k = 0; k < n_rec; k += kBatch) {
+      float2 ml[kBatch];
+      float4 o[kBatch];
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        const int64_t rec = rec0 + (int64_t)min(k + u, n_rec - 1) * stride;
-        ml[u] = p.part_ml[rec * kBlockM + r];
-        o[u] = reinterpret_cast<const float4*>(p.part_o)[(rec * (D / 4) + q4) * kBlockM + r];
-        if (k + u >= n_rec) ml[u] = make_float2(-INFINITY, 0.f);
+      for (int u = 0; u < kBatch; ++u) {
+        ml[u] = make_float2(-INFINITY, 0.f);
+        o[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (k + u < n_rec) {
+          const int64_t rec = rec0 + (int64_t)(k + u) * stride;
+          ml[u] = p.part_ml[rec * kBlockM + r];
+          o[u] = reinterpret_cast<const float4*>(p.part_o)[(rec * (D / 4) + q4) * kBlockM + r];
+        }
       }
-      const float M_new = fmaxf(fmaxf(M, fmaxf(ml[0].x, ml[1].x)), fmaxf(ml[2].x, ml[3].x));
+      float M_new = M;
+#pragma unroll
+      for (int u = 0; u < kBatch; ++u) M_new = fmaxf(M_new, ml[u].x);
       if (M_new > -INFINITY) {
         const float f = ptx::ex2(M - M_new);  // 0 while nothing has been merged yet (M = -inf)
         acc.x *= f; acc.y *= f; acc.z *= f; acc.w *= f;
         L *= f;
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
+        for (int u = 0; u < kBatch; ++u) {
           if (ml[u].x == -INFINITY) continue;  // a partial that saw no key: weight 0, accumulator not meaningful
           const float wgt = ptx::ex2(ml[u].x - M_new);
           acc.x += wgt * o[u].x; acc.y += wgt * o[u].y; acc.z += wgt * o[u].z; acc.w += wgt * o[u].w;
@@ -922,6 +931,42 @@ int64_t build_unit_prefix(Params& prm, const ws_block_mask* mask, int32_t Lq, in
   return Tp;
 }
 
+// Cost model of the schedule, in hundredths of an iteration (measured on B200 with a device-side clock trace,
+// profiles/r02_attn_schedule.md): every segment a CTA starts costs about two iterations (Q load and the first Q.K^T
+// before any softmax can run, accumulator read-out at the end).  An iteration of a single unit moves two separate K/V
+// tiles instead of one shared one; its extra cost was within the noise of the fit (cfg4: 1.58 vs 1.57 us), so both
+// kinds of iteration count the same.
+constexpr int64_t kCostPairIter = 100, kCostSingleIter = 100, kCostSegment = 200;
+
+// Contiguous partition of the flattened iterations [t_begin, T) over the CTAs such that no CTA's cost (its phase-1
+// cost p1cost[c] plus segment and iteration costs of its share) exceeds `budget`.  Fills begin[0..G] and returns
+// whether everything fitted.
+bool partition_pool(const Params& prm, int64_t Tp, int64_t t_begin, int64_t T, int64_t G, const int64_t* p1cost, int64_t budget,
+                    int64_t* begin) {
+  const int n_units = prm.n_units;
+  int64_t t = t_begin;
+  for (int64_t c = 0; c < G; ++c) {
+    begin[c] = t;
+    int64_t left = budget - p1cost[c];
+    while (t < T) {
+      const int64_t rem = t % Tp;
+      int u = 0;
+      while (u + 1 < n_units && prm.unit_prefix[u + 1] <= rem) ++u;  // unit holding rem (empty units have no iterations)
+      while (prm.unit_prefix[u + 1] == prm.unit_prefix[u]) ++u;
+      const int64_t per_iter = (prm.last_single && u == n_units - 1) ? kCostSingleIter : kCostPairIter;
+      const int64_t in_unit = prm.unit_prefix[u + 1] - rem;
+      if (left < kCostSegment + per_iter) break;
+      left -= kCostSegment;
+      const int64_t n = left / per_iter < in_unit ? left / per_iter : in_unit;
+      t += n;
+      left -= n * per_iter;
+      if (n < in_unit) break;
+    }
+  }
+  begin[G] = t;
+  return t == T;
+}
+
 // The two-phase schedule (see Params) for a device with `sms` SMs: fills prm.grid, n_waves, pool_begin.
 void build_schedule(Params& prm, int64_t Tp, int sms) {
   const int n_units = prm.n_units, H = prm.H;
@@ -930,42 +975,113 @@ void build_schedule(Params& prm, int64_t Tp, int sms) {
   if (G > sms) G = sms;
   if (G > kMaxCtas) G = kMaxCtas;
   prm.grid = (int32_t)G;
-  auto item_len = [&](int64_t i) { const int u = (int)(i % n_units); return (int64_t)(prm.unit_prefix[u + 1] - prm.unit_prefix[u]); };
+  if (T == 0) {  // nothing visible anywhere: every item is a (zero-filling) phase-1 item
+    prm.n_waves = (int32_t)((n_items + G - 1) / G);
+    for (int64_t c = 0; c <= G; ++c) prm.pool_begin[c] = 0;
+    return;
+  }
+  auto item_cost = [&](int64_t i) {
+    const int u = (int)(i % n_units);
+    const int64_t n = prm.unit_prefix[u + 1] - prm.unit_prefix[u];
+    return n == 0 ? (int64_t)0 : kCostSegment + n * ((prm.last_single && u == n_units - 1) ? kCostSingleIter : kCostPairIter);
+  };
   auto item_flat = [&](int64_t i) { return (i / n_units) * Tp + prm.unit_prefix[i % n_units]; };
-  // candidate B: W whole-item waves, the remaining items water-filled over the CTAs
+  // smallest per-CTA budget for which the pool [t_begin, T) fits next to the phase-1 costs
+  auto min_budget = [&](int64_t t_begin, const int64_t* p1cost, int64_t* begin) {
+    int64_t lo = 0, hi = 0;
+    for (int64_t c = 0; c < G; ++c) lo = p1cost[c] > lo ? p1cost[c] : lo;
+    hi = lo + (T - t_begin) * kCostSingleIter + kCostSegment * (n_items + 1) + 1;
+    while (lo < hi) {
+      const int64_t mid = (lo + hi) / 2;
+      if (partition_pool(prm, Tp, t_begin, T, G, p1cost, mid, begin)) hi = mid; else lo = mid + 1;
+    }
+    partition_pool(prm, Tp, t_begin, T, G, p1cost, lo, begin);
+    return lo;
+  };
+  int64_t zero[kMaxCtas] = {}, p1cost[kMaxCtas] = {}, begin_a[kMaxCtas + 1], begin_b[kMaxCtas + 1];
+  // candidate A: pure stream-K over all items.  The even split in iterations is kept unless the cost-aware partition
+  // (which shortens the share of CTAs that start more segments or run single-unit iterations) models > 5 % faster:
+  // with long segments the even split was measured marginally better (cfg4), with short ones clearly worse (cfg2).
+  int64_t makespan_a = min_budget(0, zero, begin_a);
+  {
+    int64_t even[kMaxCtas + 1], worst = 0;
+    for (int64_t c = 0; c <= G; ++c) even[c] = (c * T) / G;
+    for (int64_t c = 0; c < G; ++c) {
+      int64_t cost = 0;
+      for (int64_t t = even[c]; t < even[c + 1];) {
+        const int64_t rem = t % Tp;
+        int u = 0;
+        while (u + 1 < n_units && prm.unit_prefix[u + 1] <= rem) ++u;
+        while (prm.unit_prefix[u + 1] == prm.unit_prefix[u]) ++u;
+        const int64_t in_unit = prm.unit_prefix[u + 1] - rem, n = in_unit < even[c + 1] - t ? in_unit : even[c + 1] - t;
+        cost += kCostSegment + n * ((prm.last_single && u == n_units - 1) ? kCostSingleIter : kCostPairIter);
+        t += n;
+      }
+      worst = cost > worst ? cost : worst;
+    }
+    if (makespan_a * 105 >= worst * 100) {
+      makespan_a = worst;
+      for (int64_t c = 0; c <= G; ++c) begin_a[c] = even[c];
+    }
+  }
+  // candidate B: W whole-item waves, the remaining items pooled
   const int64_t W = n_items / G;
-  int64_t p1[kMaxCtas], quota[kMaxCtas];
-  int64_t pool = T, p1_max = 0;
-  for (int64_t c = 0; c < G; ++c) {
-    p1[c] = 0;
-    for (int64_t w = 0; w < W; ++w) p1[c] += item_len(w * G + c);
-    pool -= p1[c];
-    if (p1[c] > p1_max) p1_max = p1[c];
+  bool use_b = false;
+  if (W > 0) {
+    for (int64_t c = 0; c < G; ++c)
+      for (int64_t w = 0; w < W; ++w) p1cost[c] += item_cost(w * G + c);
+    const int64_t makespan_b = min_budget(item_flat(W * G), p1cost, begin_b);
+    // B trades a slightly longer critical path for far fewer split items and L2 reuse of K/V across the units of a head
+    use_b = makespan_b * 100 <= makespan_a * 103;
   }
-  // smallest level with sum_c max(0, level - p1[c]) >= pool
-  int64_t lo = 0, hi = p1_max + pool;
-  while (lo < hi) {
-    const int64_t mid = (lo + hi) / 2;
-    int64_t cap = 0;
-    for (int64_t c = 0; c < G; ++c) cap += mid > p1[c] ? mid - p1[c] : 0;
-    if (cap >= pool) hi = mid; else lo = mid + 1;
+  prm.n_waves = use_b ? (int32_t)W : 0;
+  for (int64_t c = 0; c <= G; ++c) prm.pool_begin[c] = use_b ? begin_b[c] : begin_a[c];
+}
+
+// The schedule depends on the problem shape only (Lq, H, cache_len, Ln, mask, SM count): a streaming session repeats
+// the same shape for every layer and denoising step, so the last few schedules are kept (per host thread).
+struct ScheduleKey {
+  int32_t Lq, H, Ln, n_blocks, sms;
+  int64_t cache_len;
+  int32_t q_block_end[WS_MAX_MASK_BLOCKS], kv_visible[WS_MAX_MASK_BLOCKS];
+};
+struct ScheduleEntry {
+  bool valid = false;
+  uint64_t stamp = 0;
+  ScheduleKey key;
+  int32_t n_cache_tiles, last_single, last_kv_tiles, n_waves, grid;
+  int32_t unit_prefix[kMaxUnits + 1];
+  int64_t pool_begin[kMaxCtas + 1];
+};
+// Fills the schedule fields of prm (needs Lq, H, Ln, cache_len, n_units set); returns the iterations per head.
+int64_t schedule_for(Params& prm, const ws_block_mask* mask, int sms) {
+  constexpr int kEntries = 8;
+  thread_local ScheduleEntry cache[kEntries];
+  thread_local uint64_t clock = 0;
+  ScheduleKey key;
+  memset(&key, 0, sizeof(key));
+  key.Lq = prm.Lq; key.H = prm.H; key.Ln = prm.Ln; key.n_blocks = mask->n_blocks; key.sms = sms; key.cache_len = prm.cache_len;
+  for (int b = 0; b < mask->n_blocks; ++b) { key.q_block_end[b] = mask->q_block_end[b]; key.kv_visible[b] = mask->kv_visible[b]; }
+  ScheduleEntry* victim = &cache[0];
+  for (ScheduleEntry& e : cache) {
+    if (e.valid && memcmp(&e.key, &key, sizeof(key)) == 0) {
+      e.stamp = ++clock;
+      prm.n_cache_tiles = e.n_cache_tiles; prm.last_single = e.last_single; prm.last_kv_tiles = e.last_kv_tiles;
+      prm.n_waves = e.n_waves; prm.grid = e.grid;
+      memcpy(prm.unit_prefix, e.unit_prefix, sizeof(int32_t) * (prm.n_units + 1));
+      memcpy(prm.pool_begin, e.pool_begin, sizeof(int64_t) * (e.grid + 1));
+      return prm.unit_prefix[prm.n_units];
+    }
+    if (!e.valid || e.stamp < victim->stamp || (victim->valid && !e.valid)) victim = &e;
   }
-  int64_t excess = -pool;
-  for (int64_t c = 0; c < G; ++c) { quota[c] = lo > p1[c] ? lo - p1[c] : 0; excess += quota[c]; }
-  for (int64_t c = G - 1; c >= 0 && excess > 0; --c)
-    if (quota[c] > 0) { --quota[c]; --excess; }
-  const int64_t makespan_b = lo > p1_max ? lo : p1_max, makespan_a = (T + G - 1) / G;
-  // B trades a slightly longer critical path for far fewer split items and L2 reuse of K/V across the units of a head
-  const bool use_b = W > 0 && makespan_b * 100 <= makespan_a * 103;
-  if (use_b) {
-    prm.n_waves = (int32_t)W;
-    int64_t t = item_flat(W * G);
-    for (int64_t c = 0; c < G; ++c) { prm.pool_begin[c] = t; t += quota[c]; }
-    prm.pool_begin[G] = t;  // == T
-  } else {
-    prm.n_waves = 0;
-    for (int64_t c = 0; c <= G; ++c) prm.pool_begin[c] = (c * T) / G;
-  }
+  const int64_t Tp = build_unit_prefix(prm, mask, prm.Lq, prm.cache_len, nullptr);
+  build_schedule(prm, Tp, sms);
+  victim->valid = true; victim->stamp = ++clock; victim->key = key;
+  victim->n_cache_tiles = prm.n_cache_tiles; victim->last_single = prm.last_single; victim->last_kv_tiles = prm.last_kv_tiles;
+  victim->n_waves = prm.n_waves; victim->grid = prm.grid;
+  memcpy(victim->unit_prefix, prm.unit_prefix, sizeof(int32_t) * (prm.n_units + 1));
+  memcpy(victim->pool_begin, prm.pool_begin, sizeof(int64_t) * (prm.grid + 1));
+  return Tp;
 }
 
 // The mask rules shared by the attention entry points and the schedule diagnostic.
@@ -1088,8 +1204,7 @@ int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const v
     prm.q_block_end[b] = mask->q_block_end[b];
     prm.kv_visible[b] = mask->kv_visible[b];
   }
-  const int64_t Tp = build_unit_prefix(prm, mask, Lq, cache_len, nullptr);
-  build_schedule(prm, Tp, dev->sms);
+  schedule_for(prm, mask, dev->sms);
 
   // ---- launches ----
   if (f32) {
