@@ -13,6 +13,8 @@
  *                                                                   PAPER.md:25, :73, :79
  *   ws_block_causal_attn_seq_layout   the two relayouts folded into the attention call (strided TMA)
  *   ws_seq_to_head_multi / ws_head_to_seq_multi   several same-shaped tensors in one launch
+ *   ws_kv_cache_write_fp8 / ws_block_causal_attn_fp8kv   the same cache held as FP8 (E4M3 codes and one
+ *                           power-of-two scale per (row, head)): half the bytes of the full-history cache
  *   ws_unit_forward_host   the same path for one unit fed from HOST buffers (end-to-end entry)
  *   ws_attn_schedule       host-only diagnostic: the attention work schedule for a given SM count
  *
@@ -181,6 +183,37 @@ int ws_block_causal_attn_seq_layout(void* out_seq, float* lse, const void* q_seq
                                     const void* v_new_seq, int32_t Ln, int32_t H_total, int32_t head_begin, int32_t H,
                                     int32_t d, int32_t Lq, const ws_block_mask* mask, float softmax_scale,
                                     void* workspace, size_t workspace_bytes, ws_dtype dt, void* stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * FP8 K/V cache ("local shards of the full-history cache")
+ *
+ *   The cache rows are stored as OCP FP8 E4M3 codes (1 sign, 4 exponent bits with bias 7, 3 mantissa bits, no
+ *   infinity, largest finite value 448) with ONE power-of-two scale 2^e per (row, head), e an int8:
+ *
+ *     amax = max_c |x[c]| over the row's d elements
+ *     e    = the smallest integer with 448 * 2^e >= amax, clamped to [-100, 7]      (amax == 0 -> e = -100)
+ *     code = round-to-nearest-even(x / 2^e) to E4M3, saturated to +-448 (reached only when e was clamped at 7,
+ *            i.e. |x| > 57344)
+ *     dequantised value = decode(code) * 2^e, exactly representable in BF16.
+ *
+ *   ws_kv_cache_write_fp8:  cache8[h, row_offset + r, :], exp[h, row_offset + r] = quantise(src[r, head_begin + h, :])
+ *   for K and V; every other byte is untouched.  BF16 sources only.
+ *     k_cache8, v_cache8 : device, uint8 [H, capacity, d]      k_exp, v_exp : device, int8 [H, capacity]
+ *     k_src, v_src       : device, BF16 [n_rows, H_src, d]
+ *   ws_block_causal_attn_fp8kv:  a3 with that cache; q, k_new, v_new, out stay BF16 [L, H, d].  The codes are
+ *   expanded to BF16 inside the SM (exactly), so the result is what ws_block_causal_attn returns on the dequantised
+ *   cache, up to the order of FP32 summation.  Workspace size as ws_block_causal_attn (WS_DTYPE_BF16).
+ *   Both: d in {64, 128}; capacity a multiple of 16 and every pointer 16-byte aligned (ALIGNMENT otherwise); the
+ *   other errors as their BF16 counterparts.
+ * ---------------------------------------------------------------------------------------------- */
+int ws_kv_cache_write_fp8(void* k_cache8, void* v_cache8, int8_t* k_exp, int8_t* v_exp, int64_t capacity, int32_t H, int32_t d,
+                          const void* k_src, const void* v_src, int32_t n_rows, int32_t H_src, int32_t head_begin,
+                          int64_t row_offset, void* stream);
+
+int ws_block_causal_attn_fp8kv(void* out, float* lse, const void* q, const void* k_cache8, const void* v_cache8,
+                               const int8_t* k_exp, const int8_t* v_exp, int64_t capacity, int64_t cache_len, const void* k_new,
+                               const void* v_new, int32_t Ln, int32_t H, int32_t d, int32_t Lq, const ws_block_mask* mask,
+                               float softmax_scale, void* workspace, size_t workspace_bytes, void* stream);
 
 /* ------------------------------------------------------------------------------------------------
  * a5. One unit end to end from HOST buffers ("receive the current K/V slice, update

@@ -22,7 +22,7 @@ _lib = None
 EXPORTS = (
     "ws_kv_cache_write", "ws_seq_to_head", "ws_head_to_seq", "ws_seq_to_head_multi", "ws_head_to_seq_multi", "ws_block_causal_attn_workspace_bytes",
     "ws_block_causal_attn", "ws_block_causal_attn_seq_layout", "ws_unit_forward_host_staging_bytes", "ws_unit_forward_host", "ws_status_string",
-    "ws_version", "ws_last_cuda_error", "ws_kernel_launch_count", "ws_attn_schedule",
+    "ws_version", "ws_last_cuda_error", "ws_kernel_launch_count", "ws_attn_schedule", "ws_kv_cache_write_fp8", "ws_block_causal_attn_fp8kv",
 )
 
 
@@ -78,6 +78,11 @@ def load():
     lib.ws_attn_schedule.argtypes = [i32, i32, i64, i32, ctypes.POINTER(_BlockMask), i32, ctypes.POINTER(i32), ctypes.POINTER(i32),
                                      ctypes.POINTER(i32), ctypes.POINTER(i32), ctypes.POINTER(i64)]
     lib.ws_attn_schedule.restype = ctypes.c_int
+    lib.ws_kv_cache_write_fp8.argtypes = [vp, vp, vp, vp, i64, i32, i32, vp, vp, i32, i32, i32, i64, vp]
+    lib.ws_kv_cache_write_fp8.restype = ctypes.c_int
+    lib.ws_block_causal_attn_fp8kv.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, i64, vp, vp, i32, i32, i32, i32, ctypes.POINTER(_BlockMask),
+                                               f32, vp, sz, vp]
+    lib.ws_block_causal_attn_fp8kv.restype = ctypes.c_int
     lib.ws_status_string.argtypes = [ctypes.c_int]
     lib.ws_status_string.restype = ctypes.c_char_p
     for fn in (lib.ws_version, lib.ws_last_cuda_error, lib.ws_kernel_launch_count):
@@ -230,6 +235,52 @@ def block_causal_attn(out, q, k_cache, v_cache, cache_len: int, k_new, v_new, q_
                                      _p(v_new), Ln, H, d, Lq, ctypes.byref(mask), float(softmax_scale), _p(workspace),
                                      workspace.numel() * workspace.element_size(), _dt(q), _stream(stream))
     _ok(rc, "ws_block_causal_attn")
+
+
+def kv_cache_write_fp8(k_cache8, v_cache8, k_exp, v_exp, k_src, v_src, head_begin: int = 0, row_offset: int = 0, stream=None):
+    """FP8 cache write (ws.h ws_kv_cache_write_fp8): cache8 uint8 [H, capacity, d], exp int8 [H, capacity], src BF16 [n_rows, H_src, d]."""
+    _dev(k_cache8, v_cache8, k_exp, v_exp, k_src, v_src)
+    H, capacity, d = k_cache8.shape
+    n_rows, H_src, d2 = k_src.shape
+    if d2 != d or v_cache8.shape != k_cache8.shape or v_src.shape != k_src.shape or tuple(k_exp.shape) != (H, capacity) or \
+            v_exp.shape != k_exp.shape:
+        raise ValueError("ws_kv_cache_write_fp8: shape mismatch")
+    if k_cache8.dtype != torch.uint8 or v_cache8.dtype != torch.uint8 or k_exp.dtype != torch.int8 or v_exp.dtype != torch.int8 or \
+            k_src.dtype != torch.bfloat16 or v_src.dtype != torch.bfloat16:
+        raise TypeError("ws_kv_cache_write_fp8: caches uint8, exponents int8, sources bfloat16")
+    rc = load().ws_kv_cache_write_fp8(_p(k_cache8), _p(v_cache8), _p(k_exp), _p(v_exp), capacity, H, d, _p(k_src), _p(v_src), n_rows,
+                                      H_src, head_begin, row_offset, _stream(stream))
+    _ok(rc, "ws_kv_cache_write_fp8")
+
+
+def block_causal_attn_fp8kv(out, q, k_cache8, v_cache8, k_exp, v_exp, cache_len: int, k_new, v_new, q_block_end: Sequence[int],
+                            kv_visible: Sequence[int], softmax_scale: float, workspace, lse=None, stream=None):
+    """Block-causal unit attention on an FP8 cache (ws.h ws_block_causal_attn_fp8kv); q/out/k_new/v_new BF16."""
+    _dev(out, q, k_cache8, v_cache8, k_exp, v_exp, k_new, v_new, workspace, lse)
+    Lq, H, d = q.shape
+    capacity = k_cache8.shape[1]
+    Ln = 0 if k_new is None else k_new.shape[0]
+    if out.shape != q.shape or out.dtype != q.dtype or q.dtype != torch.bfloat16:
+        raise ValueError("ws_block_causal_attn_fp8kv: out must match q (bfloat16)")
+    if tuple(k_cache8.shape) != (H, capacity, d) or v_cache8.shape != k_cache8.shape or tuple(k_exp.shape) != (H, capacity) or \
+            v_exp.shape != k_exp.shape or k_cache8.dtype != torch.uint8 or v_cache8.dtype != torch.uint8 or \
+            k_exp.dtype != torch.int8 or v_exp.dtype != torch.int8:
+        raise ValueError("ws_block_causal_attn_fp8kv: cache uint8 [H, capacity, d], exponents int8 [H, capacity]")
+    if k_new is not None and (tuple(k_new.shape) != (Ln, H, d) or v_new is None or v_new.shape != k_new.shape or
+                              k_new.dtype != q.dtype or v_new.dtype != q.dtype):
+        raise ValueError("ws_block_causal_attn_fp8kv: k_new/v_new must be bfloat16 [Ln, H, d]")
+    if lse is not None and (lse.dtype != torch.float32 or tuple(lse.shape) != (H, Lq)):
+        raise ValueError("ws_block_causal_attn_fp8kv: lse must be float32 [H, Lq]")
+    n = len(q_block_end)
+    if len(kv_visible) != n:
+        raise ValueError("ws_block_causal_attn_fp8kv: mask arrays differ in length")
+    qe = (ctypes.c_int32 * n)(*[int(x) for x in q_block_end])
+    kv = (ctypes.c_int32 * n)(*[int(x) for x in kv_visible])
+    mask = _BlockMask(n, qe, kv)
+    rc = load().ws_block_causal_attn_fp8kv(_p(out), _p(lse), _p(q), _p(k_cache8), _p(v_cache8), _p(k_exp), _p(v_exp), capacity,
+                                           int(cache_len), _p(k_new), _p(v_new), Ln, H, d, Lq, ctypes.byref(mask), float(softmax_scale),
+                                           _p(workspace), workspace.numel() * workspace.element_size(), _stream(stream))
+    _ok(rc, "ws_block_causal_attn_fp8kv")
 
 
 def block_causal_attn_seq_layout(out_seq, q_seq, k_cache, v_cache, cache_len: int, k_new_seq, v_new_seq, head_begin: int,

@@ -37,7 +37,8 @@ namespace {
 constexpr int kBlockM = 128;  // query rows per tile (one TMEM lane each)
 constexpr int kBlockN = 128;  // keys per tile
 constexpr int kPairM = 2 * kBlockM;
-constexpr int kStages = 5;    // K/V ring slots
+constexpr int kMaxStages = 5; // K/V ring slots (BF16 cache: 5; FP8 cache: 4 + a two-slot staging ring of raw FP8 tiles)
+constexpr int kStg = 2;       // FP8 staging slots
 // P is handed to the MMA warp in chunks; chunk c covers the 16-key units [chunk16(c), chunk16(c + 1)) of the tile.
 // WS_CHUNK_ENDS lists the chunk ends as decimal digits (2468 = four chunks of 32 keys; 478 = 64 + 48 + 16 keys; the last digit is 8).
 // A small LAST chunk shortens what follows the final hand-off on the critical path (its P.V, then the next Q.K^T).
@@ -63,7 +64,8 @@ __host__ __device__ constexpr int chunk_ending_at(int u) {
   return -1;
 }
 static_assert(chunk16(0) == 0 && chunk16(kPChunks) == 8, "chunks cover the 128 keys of a tile");
-constexpr int kThreads = 384; // warp 0 TMA, warp 1 MMA, warp 2 TMEM alloc, warp 3 idle, warps 4-7 / 8-11 softmax
+constexpr int kThreads = 384;  // warp 0 TMA, warp 1 MMA, warp 2 TMEM alloc, warp 3 idle, warps 4-7 / 8-11 softmax
+constexpr int kThreads8 = 512; // FP8 cache: a fourth warpgroup (warps 12-15, one per SM sub-partition) turns the raw FP8 tiles into BF16 operand tiles
 constexpr int kMaxUnits = 256;  // work units (Q-tile pairs, plus one single tile) per head
 constexpr int kMaxCtas = 256; // upper bound on the persistent grid (workspace sizing)
 constexpr int kTmemCols = 512;
@@ -85,6 +87,9 @@ struct alignas(64) Params {
   float* lse;
   float* part_o;   // [records][d/4][128][4]
   float2* part_ml; // [records][128] (m * scale * log2e, l)
+  const int8_t* k_exp;  // FP8 cache only: int8 [H, capacity] power-of-two scale exponents of the cache rows
+  const int8_t* v_exp;
+  int64_t capacity;
   int64_t cache_len;
   int64_t out_pitch;  // elements between consecutive tokens of `out` (H * d, or H_total * d for the token-major rank view)
   int32_t Lq, H, Ln, n_blocks, n_units, n_cache_tiles;
@@ -212,31 +217,38 @@ __device__ __forceinline__ SlotPlan plan_of(const Params& p, const Segment& g) {
 // ---------------------------------------------------------------------------------------------
 // the attention kernel
 // ---------------------------------------------------------------------------------------------
-template <int D>
+template <int D, bool KV8 = false>
 struct Cfg {
+  static constexpr int kStages = KV8 ? 4 : 5;             // BF16 operand ring
   static constexpr int kAtoms = D / 64;                   // 64-element (128-byte) swizzle atoms along d
   static constexpr int kAtomBytes = kBlockN * 128;        // [128 rows][128 B]
   static constexpr int kTileBytes = kAtoms * kAtomBytes;  // one Q tile == one K or V tile
   static constexpr int kSmemQ = 2 * kTileBytes;
   static constexpr int kSmemKV = kStages * kTileBytes;
+  static constexpr int kRawTileBytes = kBlockN * D;       // FP8 tile: [128 rows][D bytes], row-major, no swizzle
+  static constexpr int kRawSlotBytes = kRawTileBytes + 256;  // + the 128 scale exponents of its rows
+  static constexpr int kSmemRaw = KV8 ? kStg * kRawSlotBytes : 0;
   static constexpr int kSmemMerge = kBlockM * 8;           // (m, l) of slot 1 for the in-CTA merge of a single unit
-  static constexpr int kSmemBytes = kSmemQ + kSmemKV + 256 /*barriers*/ + kSmemMerge;
+  static constexpr int kSmemBytes = kSmemQ + kSmemKV + kSmemRaw + 256 /*barriers*/ + kSmemMerge;
   static_assert(kSmemBytes <= 227 * 1024, "shared memory budget");
+  static constexpr int kThreadsCta = KV8 ? kThreads8 : kThreads;
   static constexpr uint32_t kTmemS0 = 0, kTmemS1 = 128, kTmemO0 = 256, kTmemO1 = 256 + D;
   static constexpr uint32_t kIdescQK = ptx::make_idesc_bf16(kBlockM, kBlockN, false);
   static constexpr uint32_t kIdescPV = ptx::make_idesc_bf16(kBlockM, D, true);
 };
 
 struct Barriers {
-  uint64_t kv_full[kStages], kv_empty[kStages];
+  uint64_t kv_full[kMaxStages], kv_empty[kMaxStages];
+  uint64_t raw_full[kStg], raw_empty[kStg];  // FP8 cache: TMA -> conversion warps
   uint64_t q_full, q_empty;
   uint64_t s_full[2], p_ready[2][kPChunks], o_done[2];  // p_ready[t][c]: chunk c of tile t's P is in TMEM
   uint32_t tmem_base;
 };
 
-template <int D, bool OUT_F32>
-__global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_constant__ Params p) {
-  using C = Cfg<D>;
+template <int D, bool OUT_F32, bool KV8>
+__global__ void __launch_bounds__(KV8 ? kThreads8 : kThreads, 1) attn_fwd_kernel(const __grid_constant__ Params p) {
+  using C = Cfg<D, KV8>;
+  constexpr int kStages = C::kStages;
   // 1024-byte alignment is required by the 128-byte swizzle (TMA box and UMMA descriptor agree on it)
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   const uint32_t smem_base = ptx::smem_u32(smem_raw);
@@ -244,9 +256,10 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
   uint8_t* smem = smem_raw;
   const uint32_t sQ = smem_base;
   const uint32_t sKV = smem_base + C::kSmemQ;
-  Barriers& bar = *reinterpret_cast<Barriers*>(smem + C::kSmemQ + C::kSmemKV);
+  const uint32_t sRaw = smem_base + C::kSmemQ + C::kSmemKV;
+  Barriers& bar = *reinterpret_cast<Barriers*>(smem + C::kSmemQ + C::kSmemKV + C::kSmemRaw);
   static_assert(sizeof(Barriers) <= 256, "barrier block");
-  float2* merge_ml = reinterpret_cast<float2*>(smem + C::kSmemQ + C::kSmemKV + 256);
+  float2* merge_ml = reinterpret_cast<float2*>(smem + C::kSmemQ + C::kSmemKV + C::kSmemRaw + 256);
 
   // the warp index goes through a shuffle so that ptxas knows it is warp-uniform: the TMA and MMA
   // warps then run in uniform control flow and their descriptors live in uniform registers
@@ -254,8 +267,15 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < kStages; ++i) {
-      ptx::mbar_init(ptx::smem_u32(&bar.kv_full[i]), 1);
+      // FP8 cache: every operand tile is handed to the MMA warp by the 128 conversion threads
+      ptx::mbar_init(ptx::smem_u32(&bar.kv_full[i]), KV8 ? 4 * 32 : 1);
       ptx::mbar_init(ptx::smem_u32(&bar.kv_empty[i]), 1);
+    }
+    if constexpr (KV8) {
+      for (int i = 0; i < kStg; ++i) {
+        ptx::mbar_init(ptx::smem_u32(&bar.raw_full[i]), 1);
+        ptx::mbar_init(ptx::smem_u32(&bar.raw_empty[i]), 4 * 32);
+      }
     }
     ptx::mbar_init(ptx::smem_u32(&bar.q_full), 1);
     ptx::mbar_init(ptx::smem_u32(&bar.q_empty), 1);
@@ -284,7 +304,7 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
   wsi::pdl_trigger();
   wsi::pdl_wait();
 
-  if (warp < 4) {
+  if (warp < 4 || warp >= 12) {
     ptx::setmaxnreg_dec<56>();
     // Both single-issuer roles run on a WHOLE warp in uniform control flow (every lane walks the
     // schedule and waits on the barriers); only the TMA / tcgen05 instructions themselves sit under
@@ -306,12 +326,36 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
       uint32_t it = 0, seg = 0;
       auto load_kv = [&](int head, int j, bool is_v) {
         const uint32_t slot = it % kStages, ph = (it / kStages) & 1;
-        ptx::mbar_wait(ptx::smem_u32(&bar.kv_empty[slot]), ph ^ 1);
-        const uint32_t full = ptx::smem_u32(&bar.kv_full[slot]);
         const uint32_t dst = sKV + slot * C::kTileBytes;
+        const bool from_cache = j < n_cache_tiles;
+        uint32_t full;
+        if constexpr (KV8) {
+          // every tile is announced on the staging barrier; a cache tile lands in the staging slot as raw FP8 (its ring
+          // slot is claimed by the conversion warps), a tile of the unit's own BF16 rows lands directly in its ring slot
+          const uint32_t st = it % kStg;
+          ptx::mbar_wait(ptx::smem_u32(&bar.raw_empty[st]), ((it / kStg) & 1) ^ 1);
+          full = ptx::smem_u32(&bar.raw_full[st]);
+          if (from_cache) {
+            const uint32_t raw = sRaw + st * C::kRawSlotBytes;
+            const int64_t rows_left = p.capacity - (int64_t)j * kBlockN;
+            const uint32_t n_exp = (uint32_t)(rows_left < kBlockN ? rows_left : kBlockN);  // capacity is a multiple of 16
+            if (ptx::elect_one()) {
+              ptx::mbar_arrive_expect_tx(full, C::kRawTileBytes + n_exp);
+              ptx::tma_load_3d(raw, is_v ? (const void*)&p.map_vc : (const void*)&p.map_kc, full, 0, j * kBlockN, head);
+              ptx::bulk_load(raw + C::kRawTileBytes, (is_v ? p.v_exp : p.k_exp) + (int64_t)head * p.capacity + (int64_t)j * kBlockN, n_exp, full);
+            }
+            __syncwarp();
+            ++it;
+            return;
+          }
+          ptx::mbar_wait(ptx::smem_u32(&bar.kv_empty[slot]), ph ^ 1);
+        } else {
+          ptx::mbar_wait(ptx::smem_u32(&bar.kv_empty[slot]), ph ^ 1);
+          full = ptx::smem_u32(&bar.kv_full[slot]);
+        }
         if (ptx::elect_one()) {
           ptx::mbar_arrive_expect_tx(full, C::kTileBytes);
-          if (j < n_cache_tiles) {
+          if (from_cache) {
             const void* map = is_v ? (const void*)&p.map_vc : (const void*)&p.map_kc;
 #pragma unroll
             for (int a = 0; a < C::kAtoms; ++a) ptx::tma_load_3d(dst + a * C::kAtomBytes, map, full, a * 64, j * kBlockN, head);
@@ -452,10 +496,64 @@ __global__ void __launch_bounds__(kThreads, 1) attn_fwd_kernel(const __grid_cons
         }
         ++seg;
       }
+    } else if (KV8 && warp >= 12) {
+      // ============================== FP8 -> BF16 conversion warps ==============================
+      // Walk the tiles in the TMA producer's order.  A cache tile: raw E4M3 bytes [128 rows][D] plus the rows' scale
+      // exponents sit in the staging slot; code b of a row with exponent e becomes the BF16 number
+      // decode(b) * 2^e, written into the operand ring in the 128-byte-swizzled layout TMA would have produced.
+      // decode: the 7 magnitude bits of b, placed at BF16 bits [10:4], read as a BF16 number give decode(|b|) * 2^-120
+      // for normal AND subnormal codes alike, so one BF16 multiply by 2^(120 + e) finishes the job exactly.
+      if constexpr (KV8) {
+        const int t = (warp - 12) * 32 + lane;
+        constexpr int kChunksPerRow = D / 8, kChunks = kBlockN * kChunksPerRow / 128;  // 8-byte chunks; per thread
+        uint32_t it = 0;
+        auto convert = [&](int j) {
+          const uint32_t slot = it % kStages, st = it % kStg;
+          ptx::mbar_wait(ptx::smem_u32(&bar.raw_full[st]), (it / kStg) & 1);
+          if (j < n_cache_tiles) {
+            ptx::mbar_wait(ptx::smem_u32(&bar.kv_empty[slot]), ((it / kStages) & 1) ^ 1);
+            const uint32_t raw = sRaw + st * C::kRawSlotBytes, dst = sKV + slot * C::kTileBytes;
+#pragma unroll 4
+            for (int i = 0; i < kChunks; ++i) {
+              const int q = t + i * 128, row = q / kChunksPerRow, c8 = q % kChunksPerRow;
+              uint32_t w0, w1;
+              ptx::lds64(raw + row * D + c8 * 8, w0, w1);
+              int e = ptx::lds_s8(raw + C::kRawTileBytes + row);
+              e = e < -100 ? -100 : (e > 7 ? 7 : e);  // rows past the cache's end carry stale bytes: keep the factor finite
+              const uint32_t mult = (uint32_t)(247 + e) << 7, mult2 = mult | (mult << 16);
+              uint32_t o[4];
+              o[0] = ptx::e4m3x2_to_bf16x2_scaled(__byte_perm(w0, 0, 0x1404), mult2);
+              o[1] = ptx::e4m3x2_to_bf16x2_scaled(__byte_perm(w0, 0, 0x3424), mult2);
+              o[2] = ptx::e4m3x2_to_bf16x2_scaled(__byte_perm(w1, 0, 0x1404), mult2);
+              o[3] = ptx::e4m3x2_to_bf16x2_scaled(__byte_perm(w1, 0, 0x3424), mult2);
+              ptx::sts128(dst + (c8 >> 3) * C::kAtomBytes + row * 128 + (((c8 & 7) ^ (row & 7)) << 4), o);
+            }
+            ptx::fence_proxy_async();  // the tensor core reads shared memory through the async proxy
+          }
+          ptx::mbar_arrive(ptx::smem_u32(&bar.kv_full[slot]));
+          ptx::mbar_arrive(ptx::smem_u32(&bar.raw_empty[st]));
+          ++it;
+        };
+        SegWalk walk(p);
+        for (Segment g; walk.next(p, g);) {
+          const SlotPlan sp = plan_of(p, g);
+          if (sp.n_it == 0) continue;
+          convert(sp.jb[0]);
+          if (sp.single) convert(sp.jb[1]);
+          for (int k = 0; k < sp.n_it; ++k) {
+            convert(sp.jb[0] + k);
+            if (sp.single) convert(sp.jb[1] + k);
+            if (k + 1 < sp.n_it) {
+              convert(sp.jb[0] + k + 1);
+              if (sp.single) convert(sp.jb[1] + k + 1);
+            }
+          }
+        }
+      }
     }
   } else {
     // ============================== softmax warpgroups ==============================
-    ptx::setmaxnreg_inc<224>();
+    ptx::setmaxnreg_inc<KV8 ? 200 : 224>();
     const int tile = (warp - 4) >> 2;                    // 0 or 1: which tile slot of the CTA
     const int row_in_tile = ((warp & 3) << 5) | lane;    // == TMEM lane this thread may access
     const uint32_t lane_off = (uint32_t)((warp & 3) << 5) << 16;
@@ -799,6 +897,18 @@ bool encode_map(CUtensorMap* map, const void* base, uint64_t d0, uint64_t d1, ui
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// 3-D UINT8 tensor map of an FP8 cache [H, capacity, d] (valid rows [0, cache_len)), no swizzle, box = {d bytes, 128 rows, 1}.
+bool encode_map_u8(CUtensorMap* map, const void* base, uint64_t d, uint64_t rows, uint64_t H, uint64_t capacity) {
+  auto fn = get_encode_fn();
+  if (!fn) return false;
+  cuuint64_t dims[3] = {d, rows, H};
+  cuuint64_t strides[2] = {d, d * capacity};
+  cuuint32_t box[3] = {(cuuint32_t)d, kBlockN, 1};
+  cuuint32_t estr[3] = {1, 1, 1};
+  return fn(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 // Per-device state: the SM count and which kernel instantiations already carry their dynamic shared-memory
 // attribute on that device (cudaFuncSetAttribute is per device).  Indexed by cudaGetDevice(), like ws_unit.cu's pipes.
 constexpr int kMaxDevices = 64;
@@ -869,14 +979,14 @@ WsLayout ws_layout(int32_t Lq, int32_t H, int32_t d, int64_t kv_total, int64_t c
   return L;
 }
 
-template <int D, bool OUT_F32>
+template <int D, bool OUT_F32, bool KV8>
 int launch_attention(const Params& prm, DeviceState* st, cudaStream_t stream) {
-  using C = Cfg<D>;
-  const cudaError_t ae = ensure_smem_attr(st, (D == 128 ? 0 : 2) + (OUT_F32 ? 1 : 0), attn_fwd_kernel<D, OUT_F32>, C::kSmemBytes);
+  using C = Cfg<D, KV8>;
+  const cudaError_t ae = ensure_smem_attr(st, (D == 128 ? 0 : 3) + (KV8 ? 2 : (OUT_F32 ? 1 : 0)), attn_fwd_kernel<D, OUT_F32, KV8>, C::kSmemBytes);
   if (ae != cudaSuccess) return wsi::cuda_fail(ae);
   int launches = 0;
   if (prm.grid > 0) {
-    const cudaError_t e = wsi::launch_pdl(attn_fwd_kernel<D, OUT_F32>, dim3(prm.grid), dim3(kThreads), C::kSmemBytes, stream, prm);
+    const cudaError_t e = wsi::launch_pdl(attn_fwd_kernel<D, OUT_F32, KV8>, dim3(prm.grid), dim3(C::kThreadsCta), C::kSmemBytes, stream, prm);
     if (e != cudaSuccess) return wsi::cuda_fail(e);
     ++launches;
   }
@@ -1151,8 +1261,9 @@ namespace {
 int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const void* v_cache, int64_t capacity,
               int64_t cache_len, const void* k_new, const void* v_new, int32_t Ln, int32_t H, int32_t d, int32_t Lq,
               const ws_block_mask* mask, float softmax_scale, void* workspace, size_t workspace_bytes, ws_dtype dt,
-              void* stream_, int64_t tok_heads) {
+              void* stream_, int64_t tok_heads, const int8_t* k_exp = nullptr, const int8_t* v_exp = nullptr) {
   cudaStream_t stream = (cudaStream_t)stream_;
+  const bool kv8 = k_exp != nullptr;  // the cache holds E4M3 codes with per-row exponents (ws_block_causal_attn_fp8kv)
   // ---- validation, descriptors and schedule first: nothing is launched on any error ----
   if (const int rc = wsi::attn_validate(out, lse, q, k_cache, v_cache, capacity, cache_len, k_new, v_new, Ln, H, d, Lq, mask,
                                         softmax_scale, workspace, workspace_bytes, dt))
@@ -1184,10 +1295,14 @@ int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const v
                      : encode_map(&prm.map_kn, q_b, d, H, Lq, row_b, tok_b, 1, kBlockN));
   ok = ok && (Ln > 0 ? encode_map(&prm.map_vn, vn_b, d, H, Ln, row_b, tok_b, 1, kBlockN)
                      : encode_map(&prm.map_vn, q_b, d, H, Lq, row_b, tok_b, 1, kBlockN));
-  ok = ok && (cache_len > 0 ? encode_map(&prm.map_kc, kc_b, d, cache_len, H, row_b, row_b * cap_b, kBlockN, 1)
-                            : encode_map(&prm.map_kc, q_b, d, H, Lq, row_b, tok_b, 1, kBlockN));
-  ok = ok && (cache_len > 0 ? encode_map(&prm.map_vc, vc_b, d, cache_len, H, row_b, row_b * cap_b, kBlockN, 1)
-                            : encode_map(&prm.map_vc, q_b, d, H, Lq, row_b, tok_b, 1, kBlockN));
+  if (kv8 && cache_len > 0) {
+    ok = ok && encode_map_u8(&prm.map_kc, kc_b, d, cache_len, H, cap_b) && encode_map_u8(&prm.map_vc, vc_b, d, cache_len, H, cap_b);
+  } else {
+    ok = ok && (cache_len > 0 ? encode_map(&prm.map_kc, kc_b, d, cache_len, H, row_b, row_b * cap_b, kBlockN, 1)
+                              : encode_map(&prm.map_kc, q_b, d, H, Lq, row_b, tok_b, 1, kBlockN));
+    ok = ok && (cache_len > 0 ? encode_map(&prm.map_vc, vc_b, d, cache_len, H, row_b, row_b * cap_b, kBlockN, 1)
+                              : encode_map(&prm.map_vc, q_b, d, H, Lq, row_b, tok_b, 1, kBlockN));
+  }
   if (!ok) return wsi::cuda_fail(cudaErrorInvalidValue);
   prm.out = out;
   prm.out_pitch = tok_heads * d;
@@ -1195,6 +1310,9 @@ int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const v
   prm.part_o = reinterpret_cast<float*>(ws + L.part_o);
   prm.part_ml = reinterpret_cast<float2*>(ws + L.part_ml);
   prm.cache_len = cache_len;
+  prm.capacity = capacity;
+  prm.k_exp = k_exp;
+  prm.v_exp = v_exp;
   prm.Lq = Lq; prm.H = H; prm.Ln = Ln; prm.n_blocks = mask->n_blocks; prm.n_units = n_units;
   prm.n_cache_tiles = (int)((cache_len + kBlockN - 1) / kBlockN);
   prm.scale = softmax_scale;
@@ -1227,8 +1345,9 @@ int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const v
     if (launches) wsi::count_launch(launches);
     if (ce != cudaSuccess) return wsi::cuda_fail(ce);
   }
-  if (d == 128) return f32 ? launch_attention<128, true>(prm, dev, stream) : launch_attention<128, false>(prm, dev, stream);
-  return f32 ? launch_attention<64, true>(prm, dev, stream) : launch_attention<64, false>(prm, dev, stream);
+  if (kv8) return d == 128 ? launch_attention<128, false, true>(prm, dev, stream) : launch_attention<64, false, true>(prm, dev, stream);
+  if (d == 128) return f32 ? launch_attention<128, true, false>(prm, dev, stream) : launch_attention<128, false, false>(prm, dev, stream);
+  return f32 ? launch_attention<64, true, false>(prm, dev, stream) : launch_attention<64, false, false>(prm, dev, stream);
 }
 }  // namespace
 
@@ -1254,4 +1373,18 @@ extern "C" __attribute__((visibility("default"))) int ws_block_causal_attn_seq_l
   return attn_impl(out_seq ? static_cast<char*>(out_seq) + off : nullptr, lse, shift(q_seq), k_cache, v_cache, capacity, cache_len,
                    shift(k_new_seq), shift(v_new_seq), Ln, H, d, Lq, mask, softmax_scale, workspace, workspace_bytes, dt, stream,
                    H_total);
+}
+
+// a3 on an FP8 cache: the cache holds E4M3 codes and one power-of-two exponent per (row, head), written by
+// ws_kv_cache_write_fp8; the unit's own K/V stay BF16.  The codes are expanded to BF16 inside the SM, exactly, so the result is
+// BF16 attention on the dequantised cache.
+extern "C" __attribute__((visibility("default"))) int ws_block_causal_attn_fp8kv(void* out, float* lse, const void* q, const void* k_cache8, const void* v_cache8,
+                                          const int8_t* k_exp, const int8_t* v_exp, int64_t capacity, int64_t cache_len,
+                                          const void* k_new, const void* v_new, int32_t Ln, int32_t H, int32_t d, int32_t Lq,
+                                          const ws_block_mask* mask, float softmax_scale, void* workspace, size_t workspace_bytes,
+                                          void* stream) {
+  if (!k_exp || !v_exp) return WS_ERR_INVALID_ARG;
+  if (capacity % 16 != 0 || (reinterpret_cast<uintptr_t>(k_exp) & 15) || (reinterpret_cast<uintptr_t>(v_exp) & 15)) return WS_ERR_ALIGNMENT;
+  return attn_impl(out, lse, q, k_cache8, v_cache8, capacity, cache_len, k_new, v_new, Ln, H, d, Lq, mask, softmax_scale, workspace,
+                   workspace_bytes, WS_DTYPE_BF16, stream, H, k_exp, v_exp);
 }

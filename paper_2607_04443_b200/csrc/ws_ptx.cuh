@@ -70,6 +70,34 @@ __device__ __forceinline__ void tma_load_3d(uint32_t smem_dst, const void* map, 
       : "memory");
 }
 
+// 1-D bulk copy global -> shared (no tensor map): 16-byte aligned addresses, size a multiple of 16
+__device__ __forceinline__ void bulk_load(uint32_t smem_dst, const void* gsrc, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_dst), "l"(gsrc), "r"(bytes), "r"(bar)
+               : "memory");
+}
+
+// ------------------------------------------------------------------ plain shared-memory accesses by 32-bit address
+__device__ __forceinline__ void lds64(uint32_t addr, uint32_t& a, uint32_t& b) {
+  asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(a), "=r"(b) : "r"(addr));
+}
+__device__ __forceinline__ int lds_s8(uint32_t addr) {
+  int v;
+  asm volatile("ld.shared.s8 %0, [%1];" : "=r"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ void sts128(uint32_t addr, const uint32_t (&v)[4]) {
+  asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]) : "memory");
+}
+// two E4M3 codes sitting in bits [15:8] and [31:24] of t -> two BF16 numbers decode(code) * (BF16 factor mult2 / 2^120):
+// sign stays at bit 15 / 31, the 7 magnitude bits move to BF16 bits [10:4], one packed BF16 multiply applies the factor
+__device__ __forceinline__ uint32_t e4m3x2_to_bf16x2_scaled(uint32_t t, uint32_t mult2) {
+  const uint32_t bits = (t & 0x80008000u) | ((t >> 4) & 0x07f007f0u);
+  uint32_t r;
+  asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(bits), "r"(mult2));
+  return r;
+}
+
 // ------------------------------------------------------------------ tcgen05: TMEM management
 __device__ __forceinline__ void tmem_alloc(uint32_t smem_result, uint32_t ncols) {
   asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_result), "r"(ncols) : "memory");
