@@ -37,8 +37,8 @@ namespace {
 constexpr int kBlockM = 128;  // query rows per tile (one TMEM lane each)
 constexpr int kBlockN = 128;  // keys per tile
 constexpr int kPairM = 2 * kBlockM;
-constexpr int kMaxStages = 5; // K/V ring slots (BF16 cache: 5; FP8 cache: 4 + a two-slot staging ring of raw FP8 tiles)
-constexpr int kStg = 2;       // FP8 staging slots
+constexpr int kMaxStages = 5; // K/V ring slots (BF16 cache: 5; FP8 cache: 3 + a four-slot staging ring of raw FP8 tiles)
+constexpr int kStg = 4;       // FP8 staging slots: the raw tiles are half the size, so the prefetch depth in tiles stays the same
 // P is handed to the MMA warp in chunks; chunk c covers the 16-key units [chunk16(c), chunk16(c + 1)) of the tile.
 // WS_CHUNK_ENDS lists the chunk ends as decimal digits (2468 = four chunks of 32 keys; 478 = 64 + 48 + 16 keys; the last digit is 8).
 // A small LAST chunk shortens what follows the final hand-off on the critical path (its P.V, then the next Q.K^T).
@@ -219,7 +219,7 @@ __device__ __forceinline__ SlotPlan plan_of(const Params& p, const Segment& g) {
 // ---------------------------------------------------------------------------------------------
 template <int D, bool KV8 = false>
 struct Cfg {
-  static constexpr int kStages = KV8 ? 4 : 5;             // BF16 operand ring
+  static constexpr int kStages = KV8 ? 3 : 5;             // BF16 operand ring
   static constexpr int kAtoms = D / 64;                   // 64-element (128-byte) swizzle atoms along d
   static constexpr int kAtomBytes = kBlockN * 128;        // [128 rows][128 B]
   static constexpr int kTileBytes = kAtoms * kAtomBytes;  // one Q tile == one K or V tile
@@ -305,6 +305,8 @@ __global__ void __launch_bounds__(KV8 ? kThreads8 : kThreads, 1) attn_fwd_kernel
   wsi::pdl_wait();
 
   if (warp < 4 || warp >= 12) {
+    // register budget per warpgroup (FP8 cache: 512 threads x 128 at launch): TMA / MMA 56, conversion 56, softmax 2 x 200
+    // (softmax spills below 200; 88 registers and four loads in flight for the conversion warps measured slower for it)
     ptx::setmaxnreg_dec<56>();
     // Both single-issuer roles run on a WHOLE warp in uniform control flow (every lane walks the
     // schedule and waits on the barriers); only the TMA / tcgen05 instructions themselves sit under
@@ -330,25 +332,24 @@ __global__ void __launch_bounds__(KV8 ? kThreads8 : kThreads, 1) attn_fwd_kernel
         const bool from_cache = j < n_cache_tiles;
         uint32_t full;
         if constexpr (KV8) {
-          // every tile is announced on the staging barrier; a cache tile lands in the staging slot as raw FP8 (its ring
-          // slot is claimed by the conversion warps), a tile of the unit's own BF16 rows lands directly in its ring slot
+          // FP8 cache: this warp only streams the raw cache tiles into the staging ring (counter it = staging uses); the
+          // operand ring belongs to the conversion warps, which also fetch the tiles of the unit's own BF16 rows --
+          // a second agent claiming ring slots out of order could not tell ring phases apart by parity
+          if (!from_cache) return;
           const uint32_t st = it % kStg;
           ptx::mbar_wait(ptx::smem_u32(&bar.raw_empty[st]), ((it / kStg) & 1) ^ 1);
           full = ptx::smem_u32(&bar.raw_full[st]);
-          if (from_cache) {
-            const uint32_t raw = sRaw + st * C::kRawSlotBytes;
-            const int64_t rows_left = p.capacity - (int64_t)j * kBlockN;
-            const uint32_t n_exp = (uint32_t)(rows_left < kBlockN ? rows_left : kBlockN);  // capacity is a multiple of 16
-            if (ptx::elect_one()) {
-              ptx::mbar_arrive_expect_tx(full, C::kRawTileBytes + n_exp);
-              ptx::tma_load_3d(raw, is_v ? (const void*)&p.map_vc : (const void*)&p.map_kc, full, 0, j * kBlockN, head);
-              ptx::bulk_load(raw + C::kRawTileBytes, (is_v ? p.v_exp : p.k_exp) + (int64_t)head * p.capacity + (int64_t)j * kBlockN, n_exp, full);
-            }
-            __syncwarp();
-            ++it;
-            return;
+          const uint32_t raw = sRaw + st * C::kRawSlotBytes;
+          const int64_t rows_left = p.capacity - (int64_t)j * kBlockN;
+          const uint32_t n_exp = (uint32_t)(rows_left < kBlockN ? rows_left : kBlockN);  // capacity is a multiple of 16
+          if (ptx::elect_one()) {
+            ptx::mbar_arrive_expect_tx(full, C::kRawTileBytes + n_exp);
+            ptx::tma_load_3d(raw, is_v ? (const void*)&p.map_vc : (const void*)&p.map_kc, full, 0, j * kBlockN, head);
+            ptx::bulk_load(raw + C::kRawTileBytes, (is_v ? p.v_exp : p.k_exp) + (int64_t)head * p.capacity + (int64_t)j * kBlockN, n_exp, full);
           }
-          ptx::mbar_wait(ptx::smem_u32(&bar.kv_empty[slot]), ph ^ 1);
+          __syncwarp();
+          ++it;
+          return;
         } else {
           ptx::mbar_wait(ptx::smem_u32(&bar.kv_empty[slot]), ph ^ 1);
           full = ptx::smem_u32(&bar.kv_full[slot]);
@@ -504,48 +505,78 @@ __global__ void __launch_bounds__(KV8 ? kThreads8 : kThreads, 1) attn_fwd_kernel
       // decode: the 7 magnitude bits of b, placed at BF16 bits [10:4], read as a BF16 number give decode(|b|) * 2^-120
       // for normal AND subnormal codes alike, so one BF16 multiply by 2^(120 + e) finishes the job exactly.
       if constexpr (KV8) {
-        const int t = (warp - 12) * 32 + lane;
-        constexpr int kChunksPerRow = D / 8, kChunks = kBlockN * kChunksPerRow / 128;  // 8-byte chunks; per thread
-        uint32_t it = 0;
-        auto convert = [&](int j) {
-          const uint32_t slot = it % kStages, st = it % kStg;
-          ptx::mbar_wait(ptx::smem_u32(&bar.raw_full[st]), (it / kStg) & 1);
-          if (j < n_cache_tiles) {
-            ptx::mbar_wait(ptx::smem_u32(&bar.kv_empty[slot]), ((it / kStages) & 1) ^ 1);
-            const uint32_t raw = sRaw + st * C::kRawSlotBytes, dst = sKV + slot * C::kTileBytes;
-#pragma unroll 4
-            for (int i = 0; i < kChunks; ++i) {
-              const int q = t + i * 128, row = q / kChunksPerRow, c8 = q % kChunksPerRow;
-              uint32_t w0, w1;
-              ptx::lds64(raw + row * D + c8 * 8, w0, w1);
-              int e = ptx::lds_s8(raw + C::kRawTileBytes + row);
-              e = e < -100 ? -100 : (e > 7 ? 7 : e);  // rows past the cache's end carry stale bytes: keep the factor finite
-              const uint32_t mult = (uint32_t)(247 + e) << 7, mult2 = mult | (mult << 16);
-              uint32_t o[4];
-              o[0] = ptx::e4m3x2_to_bf16x2_scaled(__byte_perm(w0, 0, 0x1404), mult2);
-              o[1] = ptx::e4m3x2_to_bf16x2_scaled(__byte_perm(w0, 0, 0x3424), mult2);
-              o[2] = ptx::e4m3x2_to_bf16x2_scaled(__byte_perm(w1, 0, 0x1404), mult2);
-              o[3] = ptx::e4m3x2_to_bf16x2_scaled(__byte_perm(w1, 0, 0x3424), mult2);
-              ptx::sts128(dst + (c8 >> 3) * C::kAtomBytes + row * 128 + (((c8 & 7) ^ (row & 7)) << 4), o);
+        const int row = (warp - 12) * 32 + lane;  // one thread per tile row
+        uint32_t it = 0, it_raw = 0;  // operand-ring uses (every tile), staging uses (cache tiles)
+        auto convert = [&](int head, int j, bool is_v) {
+          const uint32_t slot = it % kStages;
+          const uint32_t full = ptx::smem_u32(&bar.kv_full[slot]);
+          ptx::mbar_wait(ptx::smem_u32(&bar.kv_empty[slot]), ((it / kStages) & 1) ^ 1);
+          ++it;
+          if (j >= n_cache_tiles) {
+            // a tile of the unit's own BF16 rows: TMA straight into the ring slot; the issuing thread's arrival carries the bytes
+            const uint32_t dstn = sKV + slot * C::kTileBytes;
+            if (warp == 12 && ptx::elect_one()) {
+              ptx::mbar_arrive_expect_tx(full, C::kTileBytes);
+              const void* map = is_v ? (const void*)&p.map_vn : (const void*)&p.map_kn;
+              const int r0 = (j - n_cache_tiles) * kBlockN;
+#pragma unroll
+              for (int a = 0; a < C::kAtoms; ++a) ptx::tma_load_3d(dstn + a * C::kAtomBytes, map, full, a * 64, head, r0);
+            } else {
+              ptx::mbar_arrive(full);
+            }
+            __syncwarp();
+            return;
+          }
+          const uint32_t st = it_raw % kStg;
+          ptx::mbar_wait(ptx::smem_u32(&bar.raw_full[st]), (it_raw / kStg) & 1);
+          ++it_raw;
+          {
+            const uint32_t raw = sRaw + st * C::kRawSlotBytes + row * D, dst = sKV + slot * C::kTileBytes + row * 128;
+            int e = ptx::lds_s8(sRaw + st * C::kRawSlotBytes + C::kRawTileBytes + row);
+            e = e < -100 ? -100 : (e > 7 ? 7 : e);  // rows past the cache's end carry stale bytes: keep the factor finite
+            const uint32_t mult = (uint32_t)(247 + e) << 7, mult2 = mult | (mult << 16);
+            // 16 codes (16 bytes) per step; the threads of a quarter-warp read different 16-byte slots of their rows
+            // (row pitch D = 128 or 64 bytes: the same slot of eight consecutive rows would share banks)
+            constexpr int kRowsPerLine = 128 / D;
+            constexpr int kBatch = 2;  // 16-byte loads in flight per thread (56 registers)
+#pragma unroll
+            for (int i0 = 0; i0 < D / 16; i0 += kBatch) {
+              uint32_t w[kBatch][4];
+#pragma unroll
+              for (int b = 0; b < kBatch; ++b) ptx::lds128(raw + (((i0 + b) ^ ((row / kRowsPerLine) & (D / 16 - 1))) << 4), w[b]);
+#pragma unroll
+              for (int b = 0; b < kBatch; ++b) {
+                const int c16 = (i0 + b) ^ ((row / kRowsPerLine) & (D / 16 - 1));
+                uint32_t o[8];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                  o[2 * k] = ptx::e4m3x2_to_bf16x2_scaled(__byte_perm(w[b][k], 0, 0x1404), mult2);
+                  o[2 * k + 1] = ptx::e4m3x2_to_bf16x2_scaled(__byte_perm(w[b][k], 0, 0x3424), mult2);
+                }
+                // BF16 columns [16 c16, 16 c16 + 16): 16-byte chunks 2 c16 and 2 c16 + 1 of the row, inside atom c16 / 4
+                const uint32_t base = dst + (c16 >> 2) * C::kAtomBytes;
+                const int ch = (c16 & 3) * 2;
+                ptx::sts128(base + (((ch) ^ (row & 7)) << 4), *reinterpret_cast<uint32_t(*)[4]>(&o[0]));
+                ptx::sts128(base + (((ch + 1) ^ (row & 7)) << 4), *reinterpret_cast<uint32_t(*)[4]>(&o[4]));
+              }
             }
             ptx::fence_proxy_async();  // the tensor core reads shared memory through the async proxy
           }
-          ptx::mbar_arrive(ptx::smem_u32(&bar.kv_full[slot]));
+          ptx::mbar_arrive(full);
           ptx::mbar_arrive(ptx::smem_u32(&bar.raw_empty[st]));
-          ++it;
         };
         SegWalk walk(p);
         for (Segment g; walk.next(p, g);) {
           const SlotPlan sp = plan_of(p, g);
           if (sp.n_it == 0) continue;
-          convert(sp.jb[0]);
-          if (sp.single) convert(sp.jb[1]);
+          convert(g.head, sp.jb[0], false);
+          if (sp.single) convert(g.head, sp.jb[1], false);
           for (int k = 0; k < sp.n_it; ++k) {
-            convert(sp.jb[0] + k);
-            if (sp.single) convert(sp.jb[1] + k);
+            convert(g.head, sp.jb[0] + k, true);
+            if (sp.single) convert(g.head, sp.jb[1] + k, true);
             if (k + 1 < sp.n_it) {
-              convert(sp.jb[0] + k + 1);
-              if (sp.single) convert(sp.jb[1] + k + 1);
+              convert(g.head, sp.jb[0] + k + 1, false);
+              if (sp.single) convert(g.head, sp.jb[1] + k + 1, false);
             }
           }
         }
