@@ -6,7 +6,7 @@
 // quantise (R17/R18): amax = max |x| over the row's d elements; e = the smallest integer with
 // 448 * 2^e >= amax, clamped to [-100, 7]; code = RN-even(x / 2^e) to OCP FP8 E4M3, saturated to +-448.
 // Roofline: HBM; algorithmic bytes per (row, head) = 2 d read + d + 1 written.  One group of d / 8 lanes per
-// (row, head): a 16-byte load per lane, the row maximum by shuffles on the BF16 bit patterns (no float math: |x| is
+// (row, head), four groups per thread with their loads issued together: a 16-byte load per lane, the row maximum by shuffles on the BF16 bit patterns (no float math: |x| is
 // monotone in its bits), the hardware FP32 -> E4M3 conversion, one 8-byte store per lane (a full 128-byte line per
 // row at d = 128).
 #include <cuda_bf16.h>
@@ -31,43 +31,60 @@ __device__ __forceinline__ uint32_t cvt_e4m3x2(float hi, float lo) {  // {lo -> 
   return r;
 }
 
+constexpr int kUnroll = 4;  // (row, head) groups per lane group: four independent 16-byte loads in flight per thread
+
 template <int D>
 __global__ void __launch_bounds__(kThreads) kv_write_fp8_kernel(const __grid_constant__ Fp8WriteArgs a) {
   constexpr int kLanes = D / 8;  // lanes per (row, head) group
+  constexpr int kGroups = kThreads / kLanes;
   wsi::pdl_trigger();
   const int which = blockIdx.y;
-  const int64_t g = (int64_t)blockIdx.x * (kThreads / kLanes) + threadIdx.x / kLanes;  // group = r * H + h: source order
   const int sub = threadIdx.x % kLanes;
-  const bool active = g < (int64_t)a.n_rows * a.H;
-  const int64_t r = active ? g / a.H : 0;
-  const int h = active ? (int)(g - r * a.H) : 0;
+  const int64_t n_groups = (int64_t)a.n_rows * a.H;
+  int64_t r[kUnroll];
+  int h[kUnroll];
+  bool active[kUnroll];
+#pragma unroll
+  for (int u = 0; u < kUnroll; ++u) {
+    const int64_t g = ((int64_t)blockIdx.x * kUnroll + u) * kGroups + threadIdx.x / kLanes;  // group = r * H + h: source order
+    active[u] = g < n_groups;
+    r[u] = active[u] ? g / a.H : 0;
+    h[u] = active[u] ? (int)(g - r[u] * a.H) : 0;
+  }
   wsi::pdl_wait();  // first global access below
-  uint4 v = make_uint4(0u, 0u, 0u, 0u);
-  if (active) v = a.src[which][(r * a.H_src + h) * kLanes + sub];
-  const uint32_t w[4] = {v.x, v.y, v.z, v.w};
-  // row maximum of |x| on the bit patterns
-  uint32_t amax = 0;
+  uint4 v[kUnroll];
 #pragma unroll
-  for (int i = 0; i < 4; ++i) amax = max(amax, max(w[i] & 0x7fffu, (w[i] >> 16) & 0x7fffu));
-#pragma unroll
-  for (int off = kLanes / 2; off > 0; off >>= 1) amax = max(amax, __shfl_xor_sync(0xffffffffu, amax, off));
-  // amax = 1.m * 2^E (BF16: 8 exponent bits, 7 mantissa bits); 448 = 1.75 * 2^8, so 448 * 2^e >= amax <=> e >= E - 8 (+ 1 if 1.m > 1.75)
-  int e = -100;
-  if ((amax >> 7) != 0) {  // a subnormal or zero maximum falls below the lower clamp
-    e = (int)(amax >> 7) - 127 - 8 + ((amax & 0x7fu) > 0x60u ? 1 : 0);
-    e = e < -100 ? -100 : (e > 7 ? 7 : e);
+  for (int u = 0; u < kUnroll; ++u) {
+    v[u] = make_uint4(0u, 0u, 0u, 0u);
+    if (active[u]) v[u] = a.src[which][(r[u] * a.H_src + h[u]) * kLanes + sub];
   }
-  const float inv = __uint_as_float((uint32_t)(127 - e) << 23);  // 2^-e, exact
-  uint32_t out[2];
 #pragma unroll
-  for (int i = 0; i < 2; ++i) {
-    const float x0 = __uint_as_float(w[2 * i] << 16) * inv, x1 = __uint_as_float(w[2 * i] & 0xffff0000u) * inv;
-    const float x2 = __uint_as_float(w[2 * i + 1] << 16) * inv, x3 = __uint_as_float(w[2 * i + 1] & 0xffff0000u) * inv;
-    out[i] = cvt_e4m3x2(x1, x0) | (cvt_e4m3x2(x3, x2) << 16);
-  }
-  if (active) {
-    a.cache[which][((int64_t)h * a.capacity + r) * kLanes + sub] = make_uint2(out[0], out[1]);
-    if (sub == 0) a.exps[which][(int64_t)h * a.capacity + r] = (int8_t)e;
+  for (int u = 0; u < kUnroll; ++u) {
+    const uint32_t w[4] = {v[u].x, v[u].y, v[u].z, v[u].w};
+    // row maximum of |x| on the bit patterns
+    uint32_t amax = 0;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) amax = max(amax, max(w[i] & 0x7fffu, (w[i] >> 16) & 0x7fffu));
+#pragma unroll
+    for (int off = kLanes / 2; off > 0; off >>= 1) amax = max(amax, __shfl_xor_sync(0xffffffffu, amax, off));
+    // amax = 1.m * 2^E (BF16: 8 exponent bits, 7 mantissa bits); 448 = 1.75 * 2^8, so 448 * 2^e >= amax <=> e >= E - 8 (+ 1 if 1.m > 1.75)
+    int e = -100;
+    if ((amax >> 7) != 0) {  // a subnormal or zero maximum falls below the lower clamp
+      e = (int)(amax >> 7) - 127 - 8 + ((amax & 0x7fu) > 0x60u ? 1 : 0);
+      e = e < -100 ? -100 : (e > 7 ? 7 : e);
+    }
+    const float inv = __uint_as_float((uint32_t)(127 - e) << 23);  // 2^-e, exact
+    uint32_t out[2];
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+      const float x0 = __uint_as_float(w[2 * i] << 16) * inv, x1 = __uint_as_float(w[2 * i] & 0xffff0000u) * inv;
+      const float x2 = __uint_as_float(w[2 * i + 1] << 16) * inv, x3 = __uint_as_float(w[2 * i + 1] & 0xffff0000u) * inv;
+      out[i] = cvt_e4m3x2(x1, x0) | (cvt_e4m3x2(x3, x2) << 16);
+    }
+    if (active[u]) {
+      a.cache[which][((int64_t)h[u] * a.capacity + r[u]) * kLanes + sub] = make_uint2(out[0], out[1]);
+      if (sub == 0) a.exps[which][(int64_t)h[u] * a.capacity + r[u]] = (int8_t)e;
+    }
   }
 }
 
@@ -95,7 +112,7 @@ extern "C" __attribute__((visibility("default"))) int ws_kv_cache_write_fp8(void
     for (int j = i + 1; j < 4; ++j)
       if (wsi::ranges_overlap(outs[i], out_bytes[i], outs[j], out_bytes[j])) return WS_ERR_OVERLAP;
   }
-  const int64_t groups = (int64_t)n_rows * H, per_cta = kThreads / (d / 8);
+  const int64_t groups = (int64_t)n_rows * H, per_cta = (int64_t)kUnroll * (kThreads / (d / 8));
   const int64_t blocks = (groups + per_cta - 1) / per_cta;
   if (blocks > 0x7fffffffLL) return WS_ERR_UNSUPPORTED;
   Fp8WriteArgs a;
