@@ -321,6 +321,16 @@ def bandwidth_aux(peaks):
     calls = [(lambda i=i: ws.head_to_seq(srcs[i % 28], dsts[i % 56], P, i % 4, 1)) for i in range(224)]
     ms = time_calls(calls, graph=True)
     res["head_to_seq_cfg4"] = {"us": ms * 1e3, "gbs": byts / ms / 1e6, "bytes": byts, "frac_hbm": byts / ms / 1e6 / peaks["hbm_gbs"]}
+    # what a PLAIN device copy of the same 9.42 MB payload costs in the same harness (the operation MEASURED_PEAKS.json's
+    # hbm_gbs times on 2 GiB): at this size a dependent launch is dominated by its fixed cost, not by bandwidth
+    flat_src = [t.view(-1)[: L * (H // P) * d] for t in srcs]
+    flat_dst = [t.view(-1) for t in dsts]
+    calls = [(lambda i=i: flat_dst[i % 56].copy_(flat_src[i % 28])) for i in range(224)]
+    ms_copy = time_calls(calls, graph=True)
+    res["plain_copy_same_bytes_as_cfg4_relayout"] = {"us": ms_copy * 1e3, "gbs": byts / ms_copy / 1e6, "bytes": byts,
+                                                     "frac_hbm": byts / ms_copy / 1e6 / peaks["hbm_gbs"], "what": "torch copy_ of 9.42 MB, same graph of 224 launches"}
+    for k in ("seq_to_head_cfg4", "head_to_seq_cfg4"):
+        res[k]["frac_of_plain_copy_same_size"] = ms_copy * 1e3 / res[k]["us"]
     # saturating variant: G = P full pack of a 32x longer sequence (1.2 GB read + 1.2 GB written)
     Lb = 3680 * 32
     src = rnd(Lb, H, d)
@@ -434,6 +444,102 @@ def attention_aux(peaks):
                                       "paper_budget_ms_per_unit_all_layers": 160.0}
         del kc, vc
     return res
+
+
+def fp8_aux(peaks):
+    """the cache held as FP8 (E4M3 + one power-of-two scale per (row, head)): cache-write GB/s and attention
+    time next to the BF16 cache on the same shapes, under CUDA graphs."""
+    import torch
+    import paper_2607_04443_b200 as ws
+    res = {}
+    g = torch.Generator(device="cuda").manual_seed(8)
+    rnd = lambda std, *s: (torch.randn(*s, generator=g, device="cuda", dtype=torch.float32) * std).to(torch.bfloat16)
+
+    def graph_ms(call, reps):
+        for _ in range(2):
+            call()
+        torch.cuda.synchronize()
+        st, cg = torch.cuda.Stream(), torch.cuda.CUDAGraph()
+        with torch.cuda.graph(cg, stream=st):
+            for _ in range(reps):
+                call()
+        cg.replay()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        best = None
+        for _ in range(3):
+            a.record()
+            cg.replay()
+            b.record()
+            torch.cuda.synchronize()
+            t = a.elapsed_time(b) / reps
+            best = t if best is None else min(best, t)
+        return best
+
+    for name in ("cfg2", "cfg3", "cfg5"):
+        cfg = wl.CONFIGS[name]
+        L, H, d, Tc, cap = cfg.Lq, cfg.H, cfg.d, cfg.cache_len, cfg.capacity
+        rows_k, rows_v = rnd(cfg.kv_std, Tc, H, d), rnd(cfg.kv_std, Tc, H, d)
+        kc8, vc8 = (torch.empty((H, cap, d), dtype=torch.uint8, device="cuda") for _ in range(2))
+        ke, ve = (torch.empty((H, cap), dtype=torch.int8, device="cuda") for _ in range(2))
+        ws.kv_cache_write_fp8(kc8, vc8, ke, ve, rows_k, rows_v, 0, 0)
+        del rows_k, rows_v
+        q, kn, vn = rnd(cfg.q_premul, L, H, d), rnd(cfg.kv_std, L, H, d), rnd(cfg.kv_std, L, H, d)
+        out = torch.empty_like(q)
+        wsp = torch.empty(ws.block_causal_attn_workspace_bytes(L, H, d, Tc + cfg.Ln), dtype=torch.uint8, device="cuda")
+        ms = graph_ms(lambda: ws.block_causal_attn_fp8kv(out, q, kc8, vc8, ke, ve, Tc, kn, vn, cfg.q_block_end, cfg.kv_visible,
+                                                         cfg.softmax_scale, wsp), 10)
+        tf = cfg.attn_flops() / ms / 1e9
+        res[name] = {"attention_ms_fp8_cache": ms, "tflops": tf, "frac_bf16_peak": tf / peaks["bf16_tflops"],
+                     "cache_bytes_fp8": 2 * H * cap * (d + 1), "cache_bytes_bf16": 2 * H * cap * d * 2}
+        del kc8, vc8, ke, ve
+    # cache write at cfg3's slice size, rotating over 64 windows of a 65536-row cache and 24 source sets
+    H, d, n, cap = 40, 128, 1024, 65536
+    kc8, vc8 = (torch.empty((H, cap, d), dtype=torch.uint8, device="cuda") for _ in range(2))
+    ke, ve = (torch.empty((H, cap), dtype=torch.int8, device="cuda") for _ in range(2))
+    srcs = [(rnd(1.0, n, H, d), rnd(1.0, n, H, d)) for _ in range(24)]
+    it = [0]
+
+    def wr():
+        i = it[0]
+        it[0] += 1
+        ws.kv_cache_write_fp8(kc8, vc8, ke, ve, srcs[i % 24][0], srcs[i % 24][1], 0, (i % 64) * n)
+    ms = graph_ms(wr, 192)
+    byts = 2 * n * H * (2 * d + d + 1)
+    res["cache_write_fp8_cfg3"] = {"us": ms * 1e3, "gbs": byts / ms / 1e6, "bytes": byts, "frac_hbm": byts / ms / 1e6 / peaks["hbm_gbs"]}
+    big = (rnd(1.0, 8192, H, d), rnd(1.0, 8192, H, d))
+    jt = [0]
+
+    def wr2():
+        i = jt[0]
+        jt[0] += 1
+        ws.kv_cache_write_fp8(kc8, vc8, ke, ve, big[0], big[1], 0, (i % 8) * 8192)
+    ms = graph_ms(wr2, 16)
+    byts = 2 * 8192 * H * (2 * d + d + 1)
+    res["cache_write_fp8_8192rows"] = {"us": ms * 1e3, "gbs": byts / ms / 1e6, "bytes": byts, "frac_hbm": byts / ms / 1e6 / peaks["hbm_gbs"]}
+    return res
+
+
+def run_fp8_kernels_only(args):
+    """cfg3 through the FP8-cache calls, for ncu: slice write + attention, args.warmup + args.steps times."""
+    import torch
+    import paper_2607_04443_b200 as ws
+    cfg = wl.CONFIGS[WORKLOAD]
+    x = wl.generate(cfg)
+    H, d, cap, Tc = cfg.H, cfg.d, cfg.capacity, cfg.cache_len
+    kc8, vc8 = (torch.zeros((H, cap, d), dtype=torch.uint8, device="cuda") for _ in range(2))
+    ke, ve = (torch.zeros((H, cap), dtype=torch.int8, device="cuda") for _ in range(2))
+    pre = lambda a: dev_bf16(np.ascontiguousarray(np.transpose(a[:, :cfg.cache_prefill], (1, 0, 2))))
+    ws.kv_cache_write_fp8(kc8, vc8, ke, ve, pre(x["k_cache"]), pre(x["v_cache"]), 0, 0)
+    ks, vs, q, kn, vn = (dev_bf16(a) for a in (x["k_slice"], x["v_slice"], x["q"][0], x["k_new"][0], x["v_new"][0]))
+    out = torch.empty_like(q)
+    wsp = torch.empty(ws.block_causal_attn_workspace_bytes(cfg.Lq, H, d, Tc + cfg.Ln), dtype=torch.uint8, device="cuda")
+    for _ in range(args.warmup + args.steps):
+        ws.kv_cache_write_fp8(kc8, vc8, ke, ve, ks, vs, 0, cfg.write_offset)
+        ws.block_causal_attn_fp8kv(out, q, kc8, vc8, ke, ve, Tc, kn, vn, cfg.q_block_end, cfg.kv_visible, cfg.softmax_scale, wsp)
+    torch.cuda.synchronize()
+    assert torch.isfinite(out.float()).all()
+    print("fp8 kernels ok")
 
 
 def cpu_oracle_sample(cfg, x, target_seconds: float = 12.0):
@@ -551,7 +657,7 @@ def run_ours(args):
         if not args.no_aux:
             del unit
             torch.cuda.empty_cache()
-            line["aux"] = {"bandwidth": bandwidth_aux(peaks), "attention": attention_aux(peaks),
+            line["aux"] = {"bandwidth": bandwidth_aux(peaks), "attention": attention_aux(peaks), "fp8_kv_cache": fp8_aux(peaks),
                            "hbm_peak_gbs": peaks["hbm_gbs"], "peak_source": peaks["_source"]}
     if rank == 0:
         print(json.dumps(line))
@@ -631,7 +737,11 @@ def main():
     ap.add_argument("--no-aux", action="store_true", help="skip the per-kernel bandwidth / other-config measurements")
     ap.add_argument("--kernels-only", action="store_true",
                     help="profiling mode: only the device-resident timed steps (no e2e, cpu_baseline or aux legs)")
+    ap.add_argument("--fp8-kernels-only", action="store_true",
+                    help="profiling mode: cfg3 with the cache held as FP8 (ws_kv_cache_write_fp8 + ws_block_causal_attn_fp8kv), a few calls, no JSON line")
     args = ap.parse_args()
+    if args.fp8_kernels_only:
+        return run_fp8_kernels_only(args)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
