@@ -657,8 +657,12 @@ def run_ours(args):
         if not args.no_aux:
             del unit
             torch.cuda.empty_cache()
-            line["aux"] = {"bandwidth": bandwidth_aux(peaks), "attention": attention_aux(peaks), "fp8_kv_cache": fp8_aux(peaks),
-                           "hbm_peak_gbs": peaks["hbm_gbs"], "peak_source": peaks["_source"]}
+            aux = {"hbm_peak_gbs": peaks["hbm_gbs"], "peak_source": peaks["_source"]}
+            for key, fn in (("attention", attention_aux), ("fp8_kv_cache", fp8_aux), ("bandwidth", bandwidth_aux)):
+                aux[key] = fn(peaks)
+                torch.cuda.synchronize()
+                torch.cuda.empty_cache()
+            line["aux"] = aux
     if rank == 0:
         print(json.dumps(line))
     if dist is not None:
