@@ -223,15 +223,17 @@ int ws_block_causal_attn_fp8kv(void* out, float* lse, const void* q, const void*
  *   ws_kv_cache_write (if n_slice_rows > 0) -> n_steps x attention (step s uses q_host[s],
  *   k_new_host[s], v_new_host[s]; the mask is the single block "all Lq rows see
  *   cache_len_after + Ln keys") -> D2H copy of every step's output into out_host[s].
- *   The unit is PCIe-bound, so the work is pipelined over four head groups (when H % 4 == 0 and
- *   H >= 8): a group's inputs travel as 2-D copies on an internal copy stream, its cache write and
- *   attention (ws_block_causal_attn_seq_layout on the group's heads) start on `stream` as soon as
- *   they have landed, and its output returns on a second internal stream.  Both helper streams
- *   (one pair per device, created on first use: the library's only lazily created global state
- *   besides the driver entry point) start after the work already queued on `stream` and are
- *   joined back into it -- also when a CUDA call fails half way -- so to the caller the call is
- *   ordered on `stream` like any other and a stream capture is never left unjoined.  Calls on the
- *   same device from several host threads are serialised for the length of the enqueue.
+ *   The unit is PCIe-bound (config 3: 50.8 MB in, 9.9 MB out against 0.27 ms of kernels), so every transfer is one
+ *   contiguous cudaMemcpyAsync on an internal copy stream, ordered  slice | Q[s] | K_new[s], V_new[s] | ...,  and the
+ *   attention of a step is split by key source: Q[s] against the CACHE starts as soon as the slice and Q[s] have landed
+ *   and runs under the transfer of the unit's own K/V; Q[s] against the unit's own rows follows, and a small kernel
+ *   merges the two (attention over a union of key sets = LSE-weighted mean of the two attentions; both partial results
+ *   are BF16, so the merged output carries one more BF16 rounding than ws_block_causal_attn's).  Outputs return on a
+ *   second internal stream.  Both helper streams (one pair per device, created on first use: the library's only lazily
+ *   created global state besides the driver entry point) start after the work already queued on `stream` and are
+ *   joined back into it -- also when a CUDA call fails half way -- so to the caller the call is ordered on `stream`
+ *   like any other and a stream capture is never left unjoined.  Calls on the same device from several host threads
+ *   are serialised for the length of the enqueue.
  *   The call does not synchronise; the caller synchronises the stream before reading out_host.
  *
  *   k_cache, v_cache : device [H, capacity, d]      (the persistent local cache)
@@ -239,8 +241,8 @@ int ws_block_causal_attn_fp8kv(void* out, float* lse, const void* q, const void*
  *                      row_offset; cache_len_after = valid rows once the slice is in
  *   q_host, k_new_host, v_new_host : host [n_steps][Lq | Ln, H, d] contiguous over steps
  *   out_host         : host [n_steps][Lq, H, d]
- *   staging          : device scratch >= ws_unit_forward_host_staging_bytes(...) (inputs, outputs,
- *                      attention workspace), 256-byte aligned
+ *   staging          : device scratch >= ws_unit_forward_host_staging_bytes(...) (inputs, outputs, the two
+ *                      partial results, attention workspace), 256-byte aligned
  *   BF16 only.  Same error rules as the calls it is made of.
  * ---------------------------------------------------------------------------------------------- */
 size_t ws_unit_forward_host_staging_bytes(int32_t Lq, int32_t Ln, int32_t H, int32_t d, int32_t n_slice_rows,

@@ -1073,7 +1073,7 @@ int64_t build_unit_prefix(Params& prm, const ws_block_mask* mask, int32_t Lq, in
 }
 
 // Cost model of the schedule, in hundredths of an iteration (measured on B200 with a device-side clock trace,
-// profiles/r02_attn_schedule.md): every segment a CTA starts costs about two iterations (Q load and the first Q.K^T
+// profiles/r02_attn_ncu.md): every segment a CTA starts costs about two iterations (Q load and the first Q.K^T
 // before any softmax can run, accumulator read-out at the end).  An iteration of a single unit moves two separate K/V
 // tiles instead of one shared one; its extra cost was within the noise of the fit (cfg4: 1.58 vs 1.57 us), so both
 // kinds of iteration count the same.

@@ -1,8 +1,18 @@
 // ws_unit.cu -- ws_unit_forward_host: one streaming unit end to end from HOST buffers
-// (include/ws.h a5).  Pure orchestration: async H2D copies of the unit's inputs,
-// ws_kv_cache_write, n_steps x attention, async D2H of the outputs, pipelined over four head groups
-// so that the PCIe transfers in both directions overlap the kernels.  Every data-path step is one
-// of the library's own kernels; nothing is computed on the host.
+// (include/ws.h a5).  Orchestration of the library's own kernels around plain cudaMemcpyAsync calls:
+//
+//   copy-in stream :  K/V slice  |  Q[0]  |  K_new[0], V_new[0]  |  Q[1]  |  K_new[1], V_new[1]  | ...
+//   caller's stream:  cache write -> A[0]: attention of Q[0] against the CACHE  (while K_new / V_new are still in flight)
+//                                 -> B[0]: attention of Q[0] against the unit's own rows -> LSE-weighted merge of A and B
+//   copy-out stream:                                                                        out[0] -> host  | ...
+//
+// Every transfer is ONE contiguous copy (measured on the B200 host, PCIe Gen5 x16: 55 GB/s, against 30-44 GB/s for
+// cudaMemcpy2DAsync of any row width), and the big part of the attention -- the cached keys, 94 % of them at config 3
+// -- runs under the transfer of the unit's own K/V.  What follows the last input byte is B (970 keys), the merge and the
+// output copy.  The merge is the split-KV identity the oracle pins (attention over A u B = LSE-weighted mean of attention
+// over A and over B); nothing is computed on the host.
+#include <cuda_bf16.h>
+
 #include <mutex>
 
 #include "ws_internal.h"
@@ -11,7 +21,7 @@ namespace {
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 struct Staging {
-  size_t k_slice, v_slice, q, k_new, v_new, out, attn_ws, attn_ws_bytes, total;
+  size_t k_slice, v_slice, q, k_new, v_new, out, out_a, out_b, lse_a, lse_b, attn_ws, attn_ws_bytes, total;
 };
 
 Staging staging_layout(int32_t Lq, int32_t Ln, int32_t H, int32_t d, int32_t n_slice_rows, int64_t kv_total, int32_t n_steps) {
@@ -24,6 +34,10 @@ Staging staging_layout(int32_t Lq, int32_t Ln, int32_t H, int32_t d, int32_t n_s
   s.k_new = off; off = align_up(off + (size_t)n_steps * Ln * H * d * es, 256);
   s.v_new = off; off = align_up(off + (size_t)n_steps * Ln * H * d * es, 256);
   s.out = off; off = align_up(off + (size_t)n_steps * Lq * H * d * es, 256);
+  s.out_a = off; off = align_up(off + (size_t)Lq * H * d * es, 256);
+  s.out_b = off; off = align_up(off + (size_t)Lq * H * d * es, 256);
+  s.lse_a = off; off = align_up(off + (size_t)Lq * H * 4, 256);
+  s.lse_b = off; off = align_up(off + (size_t)Lq * H * 4, 256);
   s.attn_ws = off;
   s.attn_ws_bytes = ws_block_causal_attn_workspace_bytes(Lq, H, d, kv_total, WS_DTYPE_BF16);
   off = align_up(off + s.attn_ws_bytes, 256);
@@ -31,11 +45,43 @@ Staging staging_layout(int32_t Lq, int32_t Ln, int32_t H, int32_t d, int32_t n_s
   return s;
 }
 
+// out[i, h, :] = (w_a O_a[i, h, :] + w_b O_b[i, h, :]),  w_x = exp(lse_x[h, i] - logaddexp(lse_a, lse_b)[h, i]):
+// attention over the union of two disjoint key sets from the attention over each (natural-log LSE, [H, Lq]).
+// One thread per 8 elements (16 bytes).  A side whose LSE is -inf saw no key and gets weight 0.
+__global__ void __launch_bounds__(256) merge_two_kernel(uint4* __restrict__ out, const uint4* __restrict__ oa, const uint4* __restrict__ ob,
+                                                        const float* __restrict__ lse_a, const float* __restrict__ lse_b, int32_t Lq,
+                                                        int32_t H, int32_t d8) {
+  wsi::pdl_trigger();
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, total = (int64_t)Lq * H * d8;
+  wsi::pdl_wait();
+  if (idx >= total) return;
+  const int64_t ih = idx / d8;
+  const int i = (int)(ih / H), h = (int)(ih - (int64_t)i * H);
+  const float la = lse_a[(int64_t)h * Lq + i], lb = lse_b[(int64_t)h * Lq + i];
+  const float m = fmaxf(la, lb);
+  float wa = 0.f, wb = 0.f;
+  if (m > -INFINITY) {
+    const float ea = __expf(la - m), eb = __expf(lb - m), inv = 1.f / (ea + eb);
+    wa = ea * inv;
+    wb = eb * inv;
+  }
+  const uint4 a = oa[idx], b = ob[idx];
+  const uint32_t aw[4] = {a.x, a.y, a.z, a.w}, bw[4] = {b.x, b.y, b.z, b.w};
+  uint32_t r[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const float lo = wa * __uint_as_float(aw[k] << 16) + wb * __uint_as_float(bw[k] << 16);
+    const float hi = wa * __uint_as_float(aw[k] & 0xffff0000u) + wb * __uint_as_float(bw[k] & 0xffff0000u);
+    const __nv_bfloat162 p = __floats2bfloat162_rn(lo, hi);
+    r[k] = *reinterpret_cast<const uint32_t*>(&p);
+  }
+  out[idx] = make_uint4(r[0], r[1], r[2], r[3]);
+}
+
 // Internal helper streams and events of ws_unit_forward_host (one set per device, created on first use).
-constexpr int kGroups = 4;
 struct Pipe {
   cudaStream_t copy_in = nullptr, copy_out = nullptr;
-  cudaEvent_t fork = nullptr, join = nullptr, join_out = nullptr, in_ready[kGroups] = {}, out_ready[kGroups] = {};
+  cudaEvent_t fork = nullptr, join = nullptr, join_out = nullptr, in_ready = nullptr, out_ready = nullptr;
   std::mutex enqueue_mu;  // held while a call enqueues its work: the events above are shared by all calls on the device
 };
 Pipe* get_pipe() {
@@ -47,14 +93,13 @@ Pipe* get_pipe() {
   std::lock_guard<std::mutex> lock(mu);
   if (!ready[dev]) {
     Pipe& p = pipes[dev];
-    bool ok = cudaStreamCreateWithFlags(&p.copy_in, cudaStreamNonBlocking) == cudaSuccess &&
-              cudaStreamCreateWithFlags(&p.copy_out, cudaStreamNonBlocking) == cudaSuccess &&
-              cudaEventCreateWithFlags(&p.fork, cudaEventDisableTiming) == cudaSuccess &&
-              cudaEventCreateWithFlags(&p.join, cudaEventDisableTiming) == cudaSuccess &&
-              cudaEventCreateWithFlags(&p.join_out, cudaEventDisableTiming) == cudaSuccess;
-    for (int g = 0; g < kGroups && ok; ++g)
-      ok = cudaEventCreateWithFlags(&p.in_ready[g], cudaEventDisableTiming) == cudaSuccess &&
-           cudaEventCreateWithFlags(&p.out_ready[g], cudaEventDisableTiming) == cudaSuccess;
+    const bool ok = cudaStreamCreateWithFlags(&p.copy_in, cudaStreamNonBlocking) == cudaSuccess &&
+                    cudaStreamCreateWithFlags(&p.copy_out, cudaStreamNonBlocking) == cudaSuccess &&
+                    cudaEventCreateWithFlags(&p.fork, cudaEventDisableTiming) == cudaSuccess &&
+                    cudaEventCreateWithFlags(&p.join, cudaEventDisableTiming) == cudaSuccess &&
+                    cudaEventCreateWithFlags(&p.join_out, cudaEventDisableTiming) == cudaSuccess &&
+                    cudaEventCreateWithFlags(&p.in_ready, cudaEventDisableTiming) == cudaSuccess &&
+                    cudaEventCreateWithFlags(&p.out_ready, cudaEventDisableTiming) == cudaSuccess;
     if (!ok) return nullptr;
     ready[dev] = true;
   }
@@ -86,38 +131,29 @@ extern "C" __attribute__((visibility("default"))) int ws_unit_forward_host(void*
   const Staging s = staging_layout(Lq, Ln, H, d, n_slice_rows, cache_len_after + Ln, n_steps);
   if (!staging || staging_bytes < s.total || !wsi::aligned256(staging)) return WS_ERR_WORKSPACE;
   char* st = reinterpret_cast<char*>(staging);
-  const size_t step_q = (size_t)Lq * H * d * 2, step_n = (size_t)Ln * H * d * 2;
-  const int n_groups = (H % kGroups == 0 && H >= 2 * kGroups) ? kGroups : 1;
-  const int32_t Hg = H / n_groups;
-  const size_t row_b = (size_t)d * 2, tok_b = row_b * H, grp_b = row_b * Hg;
-  const int32_t q_end = Lq, kv_vis = (int32_t)(cache_len_after + Ln);
-  ws_block_mask mask{1, &q_end, &kv_vis};
-  for (int g = 0; g < n_groups; ++g) {
-    const char* kc_g = static_cast<const char*>(k_cache) + (size_t)g * Hg * capacity * row_b;
-    const char* vc_g = static_cast<const char*>(v_cache) + (size_t)g * Hg * capacity * row_b;
-    if (n_slice_rows > 0)
-      if (const int rc = wsi::cache_write_validate(kc_g, vc_g, capacity, Hg, d, st + s.k_slice, st + s.v_slice, n_slice_rows, H, g * Hg,
-                                                   row_offset, WS_DTYPE_BF16))
-        return rc;
-    const size_t off = (size_t)g * grp_b;
-    if (const int rc = wsi::attn_validate(st + s.out + off, nullptr, st + s.q + off, kc_g, vc_g, capacity, cache_len_after,
-                                          Ln ? st + s.k_new + off : nullptr, Ln ? st + s.v_new + off : nullptr, Ln, Hg, d, Lq, &mask,
-                                          softmax_scale, st + s.attn_ws, s.attn_ws_bytes, WS_DTYPE_BF16))
+  const size_t step_q = (size_t)Lq * H * d * 2, step_n = (size_t)Ln * H * d * 2, slice_b = (size_t)n_slice_rows * H * d * 2;
+  const bool has_cache = cache_len_after > 0, has_new = Ln > 0, both = has_cache && has_new;
+  const int32_t q_end = Lq, vis_a = (int32_t)cache_len_after, vis_b = Ln, vis_none = 0;
+  const ws_block_mask mask_a{1, &q_end, &vis_a}, mask_b{1, &q_end, &vis_b}, mask_none{1, &q_end, &vis_none};
+  float* lse_a = reinterpret_cast<float*>(st + s.lse_a);
+  float* lse_b = reinterpret_cast<float*>(st + s.lse_b);
+  if (n_slice_rows > 0)
+    if (const int rc = wsi::cache_write_validate(k_cache, v_cache, capacity, H, d, st + s.k_slice, st + s.v_slice, n_slice_rows, H, 0,
+                                                 row_offset, WS_DTYPE_BF16))
       return rc;
-  }
+  if (has_cache || !has_new)
+    if (const int rc = wsi::attn_validate(st + s.out_a, lse_a, st + s.q, k_cache, v_cache, capacity, cache_len_after, nullptr, nullptr, 0, H, d,
+                                          Lq, has_cache ? &mask_a : &mask_none, softmax_scale, st + s.attn_ws, s.attn_ws_bytes, WS_DTYPE_BF16))
+      return rc;
+  if (has_new)
+    if (const int rc = wsi::attn_validate(st + s.out_b, lse_b, st + s.q, k_cache, v_cache, capacity, 0, st + s.k_new, st + s.v_new, Ln, H, d, Lq,
+                                          &mask_b, softmax_scale, st + s.attn_ws, s.attn_ws_bytes, WS_DTYPE_BF16))
+      return rc;
 
-  // ---- pipeline over head groups ----
-  // The unit is PCIe-bound (cfg3: 50.8 MB in, 9.9 MB out against 0.27 ms of kernels).  Heads are independent, so the
-  // heads are cut into groups: group g's inputs travel as 2-D copies (one head group of every token row) on an
-  // internal copy stream, its cache write and attention run on `stream` as soon as they have landed (the fused
-  // token-major call reads the group's heads in place), and its output goes home on a second internal stream while
-  // the next groups are still arriving.  Everything is joined back into `stream` before the call returns -- also
-  // when a later step fails (WS_ERR_CUDA), so a failed call never leaves a stream capture unjoined.
   Pipe* pipe = get_pipe();
   if (!pipe) return wsi::cuda_fail(cudaErrorUnknown);
   // One set of events per device: calls on the same device are serialised on the host for the length of the enqueue.
   std::lock_guard<std::mutex> enqueue_lock(pipe->enqueue_mu);
-  // measured on cfg3 (B200, PCIe Gen5): 1 group 1.41 ms per unit, 2 -> 1.28, 4 -> 1.21, 5 -> 1.20, 8 -> 1.27
   cudaError_t e = cudaEventRecord(pipe->fork, stream);
   if (e != cudaSuccess) return wsi::cuda_fail(e);  // nothing has been forked yet
   int rc = WS_OK;
@@ -125,38 +161,57 @@ extern "C" __attribute__((visibility("default"))) int ws_unit_forward_host(void*
   const bool in_forked = e == cudaSuccess;
   if (e == cudaSuccess) e = cudaStreamWaitEvent(pipe->copy_out, pipe->fork, 0);
   const bool out_forked = in_forked && e == cudaSuccess;
-  auto h2d_group = [&](size_t dst_off, const void* src, size_t rows, int g) {
-    if (e != cudaSuccess || rows == 0) return;
-    e = cudaMemcpy2DAsync(st + dst_off + g * grp_b, tok_b, static_cast<const char*>(src) + g * grp_b, tok_b, grp_b, rows,
-                          cudaMemcpyHostToDevice, pipe->copy_in);
+  auto h2d = [&](size_t dst_off, const void* src, size_t bytes) {
+    if (e == cudaSuccess && bytes > 0) e = cudaMemcpyAsync(st + dst_off, src, bytes, cudaMemcpyHostToDevice, pipe->copy_in);
   };
-  for (int g = 0; g < n_groups && e == cudaSuccess; ++g) {
-    h2d_group(s.k_slice, k_slice_host, (size_t)n_slice_rows, g);
-    h2d_group(s.v_slice, v_slice_host, (size_t)n_slice_rows, g);
-    h2d_group(s.q, q_host, (size_t)n_steps * Lq, g);
-    h2d_group(s.k_new, k_new_host, (size_t)n_steps * Ln, g);
-    h2d_group(s.v_new, v_new_host, (size_t)n_steps * Ln, g);
-    if (e == cudaSuccess) e = cudaEventRecord(pipe->in_ready[g], pipe->copy_in);
-  }
-  for (int g = 0; g < n_groups && e == cudaSuccess && rc == WS_OK; ++g) {
-    e = cudaStreamWaitEvent(stream, pipe->in_ready[g], 0);
-    if (e != cudaSuccess) break;
-    char* kc_g = static_cast<char*>(k_cache) + (size_t)g * Hg * capacity * row_b;
-    char* vc_g = static_cast<char*>(v_cache) + (size_t)g * Hg * capacity * row_b;
-    if (n_slice_rows > 0)
-      rc = ws_kv_cache_write(kc_g, vc_g, capacity, Hg, d, st + s.k_slice, st + s.v_slice, n_slice_rows, H, g * Hg, row_offset,
-                             WS_DTYPE_BF16, stream);
-    for (int32_t step = 0; step < n_steps && rc == WS_OK; ++step)
-      rc = ws_block_causal_attn_seq_layout(st + s.out + step * step_q, nullptr, st + s.q + step * step_q, kc_g, vc_g, capacity,
-                                           cache_len_after, Ln ? st + s.k_new + step * step_n : nullptr,
-                                           Ln ? st + s.v_new + step * step_n : nullptr, Ln, H, g * Hg, Hg, d, Lq, &mask,
-                                           softmax_scale, st + s.attn_ws, s.attn_ws_bytes, WS_DTYPE_BF16, stream);
-    if (rc != WS_OK) break;
-    e = cudaEventRecord(pipe->out_ready[g], stream);
-    if (e == cudaSuccess) e = cudaStreamWaitEvent(pipe->copy_out, pipe->out_ready[g], 0);
+  // the helper stream's progress so far becomes a dependency of the caller's stream (the event is re-recorded per use:
+  // a wait refers to the record that preceded it)
+  auto inputs_arrived = [&]() {
+    if (e == cudaSuccess) e = cudaEventRecord(pipe->in_ready, pipe->copy_in);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(stream, pipe->in_ready, 0);
+  };
+  // ---- the slice and the cache write ----
+  if (n_slice_rows > 0) {
+    h2d(s.k_slice, k_slice_host, slice_b);
+    h2d(s.v_slice, v_slice_host, slice_b);
+    inputs_arrived();
     if (e == cudaSuccess)
-      e = cudaMemcpy2DAsync(static_cast<char*>(out_host) + g * grp_b, tok_b, st + s.out + g * grp_b, tok_b, grp_b, (size_t)n_steps * Lq,
-                            cudaMemcpyDeviceToHost, pipe->copy_out);
+      rc = ws_kv_cache_write(k_cache, v_cache, capacity, H, d, st + s.k_slice, st + s.v_slice, n_slice_rows, H, 0, row_offset, WS_DTYPE_BF16,
+                             stream);
+  }
+  // ---- the denoising steps ----
+  for (int32_t step = 0; step < n_steps && e == cudaSuccess && rc == WS_OK; ++step) {
+    char* q_s = st + s.q + step * step_q;
+    char* out_s = st + s.out + step * step_q;
+    h2d(s.q + step * step_q, static_cast<const char*>(q_host) + step * step_q, step_q);
+    inputs_arrived();
+    if (e != cudaSuccess) break;
+    if (has_cache || !has_new)  // A: the cached keys (or, with no key at all, the zero / -inf result)
+      rc = ws_block_causal_attn(both ? st + s.out_a : out_s, both ? lse_a : nullptr, q_s, k_cache, v_cache, capacity, cache_len_after, nullptr,
+                                nullptr, 0, H, d, Lq, has_cache ? &mask_a : &mask_none, softmax_scale, st + s.attn_ws, s.attn_ws_bytes,
+                                WS_DTYPE_BF16, stream);
+    if (has_new && rc == WS_OK) {
+      h2d(s.k_new + step * step_n, static_cast<const char*>(k_new_host) + step * step_n, step_n);
+      h2d(s.v_new + step * step_n, static_cast<const char*>(v_new_host) + step * step_n, step_n);
+      inputs_arrived();
+      if (e != cudaSuccess) break;
+      // B: the unit's own rows
+      rc = ws_block_causal_attn(both ? st + s.out_b : out_s, both ? lse_b : nullptr, q_s, k_cache, v_cache, capacity, 0,
+                                st + s.k_new + step * step_n, st + s.v_new + step * step_n, Ln, H, d, Lq, &mask_b, softmax_scale,
+                                st + s.attn_ws, s.attn_ws_bytes, WS_DTYPE_BF16, stream);
+      if (both && rc == WS_OK) {
+        const int64_t total = (int64_t)Lq * H * (d / 8);
+        e = wsi::launch_pdl(merge_two_kernel, dim3((unsigned)((total + 255) / 256)), dim3(256), 0, stream, reinterpret_cast<uint4*>(out_s),
+                            reinterpret_cast<const uint4*>(st + s.out_a), reinterpret_cast<const uint4*>(st + s.out_b),
+                            (const float*)lse_a, (const float*)lse_b, Lq, H, d / 8);
+        if (e == cudaSuccess) wsi::count_launch(1);
+      }
+    }
+    if (rc != WS_OK || e != cudaSuccess) break;
+    e = cudaEventRecord(pipe->out_ready, stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(pipe->copy_out, pipe->out_ready, 0);
+    if (e == cudaSuccess)
+      e = cudaMemcpyAsync(static_cast<char*>(out_host) + step * step_q, out_s, step_q, cudaMemcpyDeviceToHost, pipe->copy_out);
   }
   // ---- join both helper streams back into `stream`, whatever happened above ----
   cudaError_t je = cudaSuccess;

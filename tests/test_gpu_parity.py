@@ -544,9 +544,9 @@ def test_unit_forward_host_matches_oracle():
         check_attn(got[s], ref, what=f"host entry step {s}")
 
 
-def test_unit_forward_host_pipelined_over_head_groups():
-    """H = 8: ws_unit_forward_host runs as four head groups (2-D copies on the internal streams, cache write and
-    fused token-major attention per group); cache and every step's output against the oracle."""
+def test_unit_forward_host_two_steps_and_reuse_of_the_helper_streams():
+    """ws_unit_forward_host with d = 64, two steps, called twice: contiguous copies on the internal streams, cache write,
+    attention against the cache and against the unit's own rows merged by LSE; cache and every step's output against the oracle."""
     rng = np.random.default_rng(31)
     H, d, Lq, Tc0, n_w, cap, steps = 8, 64, 300, 500, 100, 700, 2
     r = lambda *s: wl.bf16_round(rng.standard_normal(s, dtype=np.float32))
@@ -612,3 +612,32 @@ def test_per_device_state_survives_device_round_trips():
                 check_attn(got, ref, what=f"device {dev}")
     finally:
         torch.cuda.set_device(0)
+
+
+@pytest.mark.parametrize("Tc0,n_w,Ln", [(0, 0, 200), (300, 0, 0), (0, 0, 0), (100, 28, 77)])
+def test_unit_forward_host_degenerate_key_sources(Tc0, n_w, Ln):
+    """No cache at all (only the unit's own rows), no own rows (only the cache), no key whatsoever (zeros), and a ragged
+    mix: the single-source cases skip the merge."""
+    rng = np.random.default_rng(33)
+    H, d, Lq, cap = 3, 128, 150, 512
+    r = lambda *s: wl.bf16_round(rng.standard_normal(s, dtype=np.float32))
+    k_cache, v_cache = np.zeros((H, cap, d), np.float32), np.zeros((H, cap, d), np.float32)
+    k_cache[:, :Tc0], v_cache[:, :Tc0] = r(H, Tc0, d), r(H, Tc0, d)
+    q = r(1, Lq, H, d)
+    kn, vn = (r(1, Ln, H, d), r(1, Ln, H, d)) if Ln else (None, None)
+    ks, vs = (r(n_w, H, d), r(n_w, H, d)) if n_w else (None, None)
+    Tc, scale = Tc0 + n_w, 1.0 / math.sqrt(d)
+    host = lambda a: None if a is None else torch.from_numpy(wl.bf16_bits(a).view(np.int16)).view(torch.bfloat16).pin_memory()
+    kc, vc = to_dev(k_cache, "bf16"), to_dev(v_cache, "bf16")
+    outh = torch.full((1, Lq, H, d), 9.0, dtype=torch.bfloat16).pin_memory()
+    staging = torch.empty(ws.unit_forward_host_staging_bytes(Lq, Ln, H, d, n_w, Tc + Ln, 1), dtype=torch.uint8, device="cuda")
+    ws.unit_forward_host(outh, host(q), host(kn), host(vn), kc, vc, host(ks), host(vs), Tc0, Tc, scale, staging)
+    torch.cuda.synchronize()
+    rk, rv = k_cache.copy(), v_cache.copy()
+    if n_w:
+        wsref.kv_cache_write(rk, rv, ks, vs, 0, Tc0)
+    got = wl.bf16_from_bits(outh.view(torch.int16).numpy().view(np.uint16))[0]
+    ref, _ = wsref.block_causal_attn(q[0], rk, rv, Tc, None if kn is None else kn[0], None if vn is None else vn[0], [Lq], [Tc + Ln], scale)
+    check_attn(got, ref, what=f"host entry Tc0={Tc0} n_w={n_w} Ln={Ln}")
+    if Tc + Ln == 0:
+        assert np.all(got == 0.0)
