@@ -15,6 +15,8 @@
  *   ws_seq_to_head_multi / ws_head_to_seq_multi   several same-shaped tensors in one launch
  *   ws_kv_cache_write_fp8 / ws_block_causal_attn_fp8kv   the same cache held as FP8 (E4M3 codes and one
  *                           power-of-two scale per (row, head)): half the bytes of the full-history cache
+ *   ws_kv_cache_write_ring / ws_block_causal_attn_ring / ws_ring_state   the cache as a sliding window over an
+ *                           unbounded session: a ring that keeps the most recent `capacity` rows
  *   ws_unit_forward_host   the same path for one unit fed from HOST buffers (end-to-end entry)
  *   ws_attn_schedule       host-only diagnostic: the attention work schedule for a given SM count
  *
@@ -214,6 +216,38 @@ int ws_block_causal_attn_fp8kv(void* out, float* lse, const void* q, const void*
                                const int8_t* k_exp, const int8_t* v_exp, int64_t capacity, int64_t cache_len, const void* k_new,
                                const void* v_new, int32_t Ln, int32_t H, int32_t d, int32_t Lq, const ws_block_mask* mask,
                                float softmax_scale, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * Ring (sliding-window) K/V cache (SURVEY.md 8(f).4 "cache windowing/eviction for unbounded sessions"
+ * "local shards of the full-history cache", PAPER.md:47 one committed unit per 160 ms without end).  The paper gives no
+ * eviction rule; reading R19:
+ *
+ *   The cache is a ring of `capacity` rows per head that keeps the MOST RECENT rows of the session.  Row w of the
+ *   session (w = 0, 1, 2, ...) lives in physical row w mod capacity until row w + capacity overwrites it.  After W rows:
+ *       cache_len = min(W, capacity),   ring_start = W < capacity ? 0 : W mod capacity      (ws_ring_state, host only)
+ *   and cache key j of the attention timeline (oldest first) is physical row (ring_start + j) mod capacity.
+ *
+ *   ws_kv_cache_write_ring:  cache[h, (write_pos + r) mod capacity, :] = src[r, head_begin + h, :] for K and V, every
+ *     other byte untouched; write_pos = rows of the session written before this call.  Arguments as ws_kv_cache_write.
+ *     Errors as ws_kv_cache_write, with OUT_OF_RANGE for write_pos < 0 or n_rows > capacity (a call never overwrites
+ *     a row it has written itself).  One launch, two when the slice wraps.
+ *   ws_block_causal_attn_ring:  ws_block_causal_attn whose cache keys are the window in timeline order; kv_visible
+ *     cuts that timeline.  The window is at most two physical runs of the cache tensor, each read in place by TMA
+ *     (no linearised copy); ring_start need not be aligned to anything.  ALL `capacity` rows of the cache tensor must hold
+ *     finite values (zero-initialise the ring before the session): a 128-row tile that straddles the window's end reads
+ *     rows outside it, which are masked out of the softmax but still multiplied by zero.  Arguments, workspace and errors as ws_block_causal_attn, plus OUT_OF_RANGE unless
+ *     0 <= ring_start < capacity.  ring_start == 0 is ws_block_causal_attn itself.
+ * ---------------------------------------------------------------------------------------------- */
+int ws_kv_cache_write_ring(void* k_cache, void* v_cache, int64_t capacity, int32_t H, int32_t d, const void* k_src,
+                           const void* v_src, int32_t n_rows, int32_t H_src, int32_t head_begin, int64_t write_pos, ws_dtype dt,
+                           void* stream);
+
+int ws_ring_state(int64_t rows_written, int64_t capacity, int64_t* ring_start /* host */, int64_t* cache_len /* host */);
+
+int ws_block_causal_attn_ring(void* out, float* lse, const void* q, const void* k_cache, const void* v_cache, int64_t capacity,
+                              int64_t ring_start, int64_t cache_len, const void* k_new, const void* v_new, int32_t Ln, int32_t H,
+                              int32_t d, int32_t Lq, const ws_block_mask* mask, float softmax_scale, void* workspace,
+                              size_t workspace_bytes, ws_dtype dt, void* stream);
 
 /* ------------------------------------------------------------------------------------------------
  * a5. One unit end to end from HOST buffers ("receive the current K/V slice, update

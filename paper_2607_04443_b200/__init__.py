@@ -10,6 +10,7 @@ from .binding import (  # noqa: F401
     kv_cache_write, seq_to_head, head_to_seq, seq_to_head_multi, head_to_seq_multi,
     block_causal_attn, block_causal_attn_workspace_bytes, block_causal_attn_seq_layout,
     kv_cache_write_fp8, block_causal_attn_fp8kv,
+    kv_cache_write_ring, block_causal_attn_ring, ring_state,
     unit_forward_host, unit_forward_host_staging_bytes, kernel_launch_count, attn_schedule, EXPORTS,
     DTYPE_BF16, DTYPE_F32,
 )

@@ -23,6 +23,7 @@ EXPORTS = (
     "ws_kv_cache_write", "ws_seq_to_head", "ws_head_to_seq", "ws_seq_to_head_multi", "ws_head_to_seq_multi", "ws_block_causal_attn_workspace_bytes",
     "ws_block_causal_attn", "ws_block_causal_attn_seq_layout", "ws_unit_forward_host_staging_bytes", "ws_unit_forward_host", "ws_status_string",
     "ws_version", "ws_last_cuda_error", "ws_kernel_launch_count", "ws_attn_schedule", "ws_kv_cache_write_fp8", "ws_block_causal_attn_fp8kv",
+    "ws_kv_cache_write_ring", "ws_ring_state", "ws_block_causal_attn_ring",
 )
 
 
@@ -83,6 +84,13 @@ def load():
     lib.ws_block_causal_attn_fp8kv.argtypes = [vp, vp, vp, vp, vp, vp, vp, i64, i64, vp, vp, i32, i32, i32, i32, ctypes.POINTER(_BlockMask),
                                                f32, vp, sz, vp]
     lib.ws_block_causal_attn_fp8kv.restype = ctypes.c_int
+    lib.ws_kv_cache_write_ring.argtypes = [vp, vp, i64, i32, i32, vp, vp, i32, i32, i32, i64, ctypes.c_int, vp]
+    lib.ws_kv_cache_write_ring.restype = ctypes.c_int
+    lib.ws_ring_state.argtypes = [i64, i64, ctypes.POINTER(i64), ctypes.POINTER(i64)]
+    lib.ws_ring_state.restype = ctypes.c_int
+    lib.ws_block_causal_attn_ring.argtypes = [vp, vp, vp, vp, vp, i64, i64, i64, vp, vp, i32, i32, i32, i32,
+                                              ctypes.POINTER(_BlockMask), f32, vp, sz, ctypes.c_int, vp]
+    lib.ws_block_causal_attn_ring.restype = ctypes.c_int
     lib.ws_status_string.argtypes = [ctypes.c_int]
     lib.ws_status_string.restype = ctypes.c_char_p
     for fn in (lib.ws_version, lib.ws_last_cuda_error, lib.ws_kernel_launch_count):
@@ -235,6 +243,58 @@ def block_causal_attn(out, q, k_cache, v_cache, cache_len: int, k_new, v_new, q_
                                      _p(v_new), Ln, H, d, Lq, ctypes.byref(mask), float(softmax_scale), _p(workspace),
                                      workspace.numel() * workspace.element_size(), _dt(q), _stream(stream))
     _ok(rc, "ws_block_causal_attn")
+
+
+def kv_cache_write_ring(k_cache, v_cache, k_src, v_src, head_begin: int = 0, write_pos: int = 0, stream=None):
+    """Ring cache write (ws.h ws_kv_cache_write_ring): cache[h, (write_pos + r) mod capacity, :] = src[r, head_begin + h, :]."""
+    _dev(k_cache, v_cache, k_src, v_src)
+    H, capacity, d = k_cache.shape
+    n_rows, H_src, d2 = k_src.shape
+    if d2 != d or v_cache.shape != k_cache.shape or v_src.shape != k_src.shape:
+        raise ValueError("ws_kv_cache_write_ring: shape mismatch")
+    if not (k_cache.dtype == v_cache.dtype == k_src.dtype == v_src.dtype):
+        raise TypeError("ws_kv_cache_write_ring: dtype mismatch")
+    rc = load().ws_kv_cache_write_ring(_p(k_cache), _p(v_cache), capacity, H, d, _p(k_src), _p(v_src), n_rows, H_src, head_begin,
+                                       int(write_pos), _dt(k_cache), _stream(stream))
+    _ok(rc, "ws_kv_cache_write_ring")
+
+
+def ring_state(rows_written: int, capacity: int):
+    """(ring_start, cache_len) of a ring cache after rows_written rows of the session (ws.h ws_ring_state; host only)."""
+    a, b = ctypes.c_int64(0), ctypes.c_int64(0)
+    _ok(load().ws_ring_state(int(rows_written), int(capacity), ctypes.byref(a), ctypes.byref(b)), "ws_ring_state")
+    return int(a.value), int(b.value)
+
+
+def block_causal_attn_ring(out, q, k_cache, v_cache, ring_start: int, cache_len: int, k_new, v_new, q_block_end: Sequence[int],
+                           kv_visible: Sequence[int], softmax_scale: float, workspace, lse=None, stream=None):
+    """Block-causal unit attention on a ring cache (ws.h ws_block_causal_attn_ring): cache key j is physical row
+    (ring_start + j) mod capacity.  Shapes as block_causal_attn."""
+    _dev(out, q, k_cache, v_cache, k_new, v_new, workspace, lse)
+    Lq, H, d = q.shape
+    capacity = k_cache.shape[1]
+    Ln = 0 if k_new is None else k_new.shape[0]
+    if out.shape != q.shape or out.dtype != q.dtype:
+        raise ValueError("ws_block_causal_attn_ring: out must match q")
+    if tuple(k_cache.shape) != (H, capacity, d) or v_cache.shape != k_cache.shape:
+        raise ValueError("ws_block_causal_attn_ring: cache must be [H, capacity, d]")
+    if k_new is not None and (tuple(k_new.shape) != (Ln, H, d) or v_new is None or v_new.shape != k_new.shape):
+        raise ValueError("ws_block_causal_attn_ring: k_new/v_new must be [Ln, H, d]")
+    for t in (k_cache, v_cache, k_new, v_new):
+        if t is not None and t.dtype != q.dtype:
+            raise TypeError("ws_block_causal_attn_ring: dtype mismatch")
+    if lse is not None and (lse.dtype != torch.float32 or tuple(lse.shape) != (H, Lq)):
+        raise ValueError("ws_block_causal_attn_ring: lse must be float32 [H, Lq]")
+    n = len(q_block_end)
+    if len(kv_visible) != n:
+        raise ValueError("ws_block_causal_attn_ring: mask arrays differ in length")
+    qe = (ctypes.c_int32 * n)(*[int(x) for x in q_block_end])
+    kv = (ctypes.c_int32 * n)(*[int(x) for x in kv_visible])
+    mask = _BlockMask(n, qe, kv)
+    rc = load().ws_block_causal_attn_ring(_p(out), _p(lse), _p(q), _p(k_cache), _p(v_cache), capacity, int(ring_start), int(cache_len),
+                                          _p(k_new), _p(v_new), Ln, H, d, Lq, ctypes.byref(mask), float(softmax_scale), _p(workspace),
+                                          workspace.numel() * workspace.element_size(), _dt(q), _stream(stream))
+    _ok(rc, "ws_block_causal_attn_ring")
 
 
 def kv_cache_write_fp8(k_cache8, v_cache8, k_exp, v_exp, k_src, v_src, head_begin: int = 0, row_offset: int = 0, stream=None):

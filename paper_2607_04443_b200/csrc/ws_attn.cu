@@ -91,6 +91,12 @@ struct alignas(64) Params {
   const int8_t* v_exp;
   int64_t capacity;
   int64_t cache_len;
+  // Ring cache (ws_block_causal_attn_ring): cache key j of the timeline is physical row (ring_start + j) mod capacity.  The
+  // window is at most two physical runs: A = rows [ring_start, ring_start + len_a) (n_tiles_a KV tiles; the last one may be
+  // partial: TMA zero-fills past the tensor's end) and B = rows [0, cache_len - len_a).  Linear cache: ring_start = 0,
+  // len_a = cache_len, n_tiles_a = n_cache_tiles.
+  int64_t ring_start, len_a;
+  int32_t n_tiles_a;
   int64_t out_pitch;  // elements between consecutive tokens of `out` (H * d, or H_total * d for the token-major rank view)
   int32_t Lq, H, Ln, n_blocks, n_units, n_cache_tiles;
   // the last unit of a head is a single Q tile (odd number of Q tiles) that sees last_kv_tiles KV tiles
@@ -358,8 +364,9 @@ __global__ void __launch_bounds__(KV8 ? kThreads8 : kThreads, 1) attn_fwd_kernel
           ptx::mbar_arrive_expect_tx(full, C::kTileBytes);
           if (from_cache) {
             const void* map = is_v ? (const void*)&p.map_vc : (const void*)&p.map_kc;
+            const int r0 = j < p.n_tiles_a ? (int)p.ring_start + j * kBlockN : (j - p.n_tiles_a) * kBlockN;  // run A / run B of a ring
 #pragma unroll
-            for (int a = 0; a < C::kAtoms; ++a) ptx::tma_load_3d(dst + a * C::kAtomBytes, map, full, a * 64, j * kBlockN, head);
+            for (int a = 0; a < C::kAtoms; ++a) ptx::tma_load_3d(dst + a * C::kAtomBytes, map, full, a * 64, r0, head);
           } else {
             const void* map = is_v ? (const void*)&p.map_vn : (const void*)&p.map_kn;
             const int r0 = (j - n_cache_tiles) * kBlockN;
@@ -646,13 +653,15 @@ __global__ void __launch_bounds__(KV8 ? kThreads8 : kThreads, 1) attn_fwd_kernel
       // sees: masking them would push their whole warp onto the slower boundary path for every tile
       const int nvis = p.kv_visible[block_of_row(p, min(row, p.Lq - 1))];
       const int vis_cache = (int)min((int64_t)nvis, p.cache_len);
+      const int vis_a = (int)min((int64_t)vis_cache, p.len_a);  // visible rows of the cache's first physical run
       float m = -INFINITY, l = 0.f;  // running max in raw-score units, running sum
       const int j_begin = tile ? sp.jb[1] : sp.jb[0];
 
       for (int k = 0; k < sp.n_it; ++k, ++n_iter) {
         const int j = j_begin + k;
         int lim;  // columns [0, lim) of this tile are visible to this row (<= 0: none; a run past the visible range)
-        if (j < p.n_cache_tiles) lim = vis_cache - j * kBlockN;
+        if (j < p.n_tiles_a) lim = vis_a - j * kBlockN;
+        else if (j < p.n_cache_tiles) lim = vis_cache - (int)p.len_a - (j - p.n_tiles_a) * kBlockN;  // second run of a ring
         else lim = nvis - (int)p.cache_len - (j - p.n_cache_tiles) * kBlockN;
 
         ptx::mbar_wait(s_full, n_iter & 1);
@@ -886,15 +895,15 @@ __global__ void __launch_bounds__(kPairM) attn_combine_kernel(const __grid_const
 }
 
 // FP32 -> BF16 staging for WS_DTYPE_F32 inputs (config 1; R9).
-// Copies `rows` rows of `row_elems` contiguous floats; source rows `src_pitch` floats apart per plane.
+// Copies n_planes planes of plane_elems contiguous floats; planes are src_plane_pitch floats / dst_plane_pitch BF16 elements apart.
 __global__ void cast_f32_to_bf16_kernel(__nv_bfloat16* __restrict__ dst, const float* __restrict__ src, int64_t n_planes,
-                                        int64_t plane_elems, int64_t src_plane_pitch) {
+                                        int64_t plane_elems, int64_t src_plane_pitch, int64_t dst_plane_pitch) {
   wsi::pdl_trigger();
   wsi::pdl_wait();
   const int64_t total = n_planes * plane_elems;
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
     const int64_t pl = i / plane_elems, e = i - pl * plane_elems;
-    dst[i] = __float2bfloat16_rn(src[pl * src_plane_pitch + e]);
+    dst[pl * dst_plane_pitch + e] = __float2bfloat16_rn(src[pl * src_plane_pitch + e]);
   }
 }
 
@@ -1039,15 +1048,32 @@ extern "C" __attribute__((visibility("default"))) size_t ws_block_causal_attn_wo
 }
 
 namespace {
+// The cache part of the key timeline as physical runs of the cache tensor (a ring's window wraps at most once): run A =
+// rows [ring_start, ring_start + len_a), run B = rows [0, cache_len - len_a).  Each run is tiled on its own (its last tile
+// may be partial), so the timeline has n_tiles_a + n_tiles_b cache tiles.  A linear cache is the case ring_start = 0.
+struct CacheRuns {
+  int64_t len_a, len_b;
+  int n_tiles_a, n_tiles_b;
+};
+CacheRuns cache_runs(int64_t capacity, int64_t ring_start, int64_t cache_len) {
+  CacheRuns r;
+  r.len_a = ring_start + cache_len <= capacity || ring_start == 0 ? cache_len : capacity - ring_start;
+  r.len_b = cache_len - r.len_a;
+  r.n_tiles_a = (int)((r.len_a + kBlockN - 1) / kBlockN);
+  r.n_tiles_b = (int)((r.len_b + kBlockN - 1) / kBlockN);
+  return r;
+}
+
 // KV tiles the last row of Q tile `qt` can see (a tile visits exactly those).
-int64_t kv_tiles_of_q_tile(const ws_block_mask* mask, int32_t Lq, int64_t cache_len, int qt) {
+int64_t kv_tiles_of_q_tile(const ws_block_mask* mask, int32_t Lq, int64_t cache_len, const CacheRuns& runs, int qt) {
   const int last_row = ((qt + 1) * kBlockM < Lq ? (qt + 1) * kBlockM : Lq) - 1;
   int b = 0;
   while (last_row >= mask->q_block_end[b]) ++b;
   const int64_t nvis = mask->kv_visible[b];
   if (nvis <= 0) return 0;
-  const int64_t nct = (cache_len + kBlockN - 1) / kBlockN;
-  return nvis <= cache_len ? (nvis + kBlockN - 1) / kBlockN : nct + (nvis - cache_len + kBlockN - 1) / kBlockN;
+  if (nvis <= runs.len_a) return (nvis + kBlockN - 1) / kBlockN;
+  if (nvis <= cache_len) return runs.n_tiles_a + (nvis - runs.len_a + kBlockN - 1) / kBlockN;
+  return runs.n_tiles_a + runs.n_tiles_b + (nvis - cache_len + kBlockN - 1) / kBlockN;
 }
 
 // Work units of a head and their iteration counts: Q tiles (2u, 2u + 1) form pair unit u, which runs one iteration
@@ -1055,7 +1081,10 @@ int64_t kv_tiles_of_q_tile(const ws_block_mask* mask, int32_t Lq, int64_t cache_
 // tile slot), i.e. one iteration per two KV tiles.  Fills prm.unit_prefix / n_cache_tiles / last_* (needs
 // prm.n_units) and returns the iterations per head.  unit_kv_tiles (optional): KV tiles each unit visits.
 int64_t build_unit_prefix(Params& prm, const ws_block_mask* mask, int32_t Lq, int64_t cache_len, int32_t* unit_kv_tiles) {
-  prm.n_cache_tiles = (int)((cache_len + kBlockN - 1) / kBlockN);
+  const CacheRuns runs = cache_runs(prm.capacity, prm.ring_start, cache_len);
+  prm.len_a = runs.len_a;
+  prm.n_tiles_a = runs.n_tiles_a;
+  prm.n_cache_tiles = runs.n_tiles_a + runs.n_tiles_b;
   const int n_q_tiles = (Lq + kBlockM - 1) / kBlockM;
   prm.last_single = n_q_tiles & 1;
   prm.last_kv_tiles = 0;
@@ -1063,7 +1092,7 @@ int64_t build_unit_prefix(Params& prm, const ws_block_mask* mask, int32_t Lq, in
   prm.unit_prefix[0] = 0;
   for (int u = 0; u < prm.n_units; ++u) {
     const bool single = prm.last_single && u == prm.n_units - 1;
-    const int64_t n = kv_tiles_of_q_tile(mask, Lq, cache_len, single ? 2 * u : 2 * u + 1);
+    const int64_t n = kv_tiles_of_q_tile(mask, Lq, cache_len, runs, single ? 2 * u : 2 * u + 1);
     if (single) prm.last_kv_tiles = (int32_t)n;
     if (unit_kv_tiles) unit_kv_tiles[u] = (int32_t)n;
     Tp += single ? (n + 1) / 2 : n;
@@ -1183,14 +1212,15 @@ void build_schedule(Params& prm, int64_t Tp, int sms) {
 // the same shape for every layer and denoising step, so the last few schedules are kept (per host thread).
 struct ScheduleKey {
   int32_t Lq, H, Ln, n_blocks, sms;
-  int64_t cache_len;
+  int64_t cache_len, capacity, ring_start;
   int32_t q_block_end[WS_MAX_MASK_BLOCKS], kv_visible[WS_MAX_MASK_BLOCKS];
 };
 struct ScheduleEntry {
   bool valid = false;
   uint64_t stamp = 0;
   ScheduleKey key;
-  int32_t n_cache_tiles, last_single, last_kv_tiles, n_waves, grid;
+  int32_t n_cache_tiles, n_tiles_a, last_single, last_kv_tiles, n_waves, grid;
+  int64_t len_a;
   int32_t unit_prefix[kMaxUnits + 1];
   int64_t pool_begin[kMaxCtas + 1];
 };
@@ -1202,12 +1232,14 @@ int64_t schedule_for(Params& prm, const ws_block_mask* mask, int sms) {
   ScheduleKey key;
   memset(&key, 0, sizeof(key));
   key.Lq = prm.Lq; key.H = prm.H; key.Ln = prm.Ln; key.n_blocks = mask->n_blocks; key.sms = sms; key.cache_len = prm.cache_len;
+  key.ring_start = prm.ring_start; key.capacity = prm.ring_start ? prm.capacity : 0;  // a linear cache's schedule does not depend on its capacity
   for (int b = 0; b < mask->n_blocks; ++b) { key.q_block_end[b] = mask->q_block_end[b]; key.kv_visible[b] = mask->kv_visible[b]; }
   ScheduleEntry* victim = &cache[0];
   for (ScheduleEntry& e : cache) {
     if (e.valid && memcmp(&e.key, &key, sizeof(key)) == 0) {
       e.stamp = ++clock;
-      prm.n_cache_tiles = e.n_cache_tiles; prm.last_single = e.last_single; prm.last_kv_tiles = e.last_kv_tiles;
+      prm.n_cache_tiles = e.n_cache_tiles; prm.n_tiles_a = e.n_tiles_a; prm.len_a = e.len_a;
+      prm.last_single = e.last_single; prm.last_kv_tiles = e.last_kv_tiles;
       prm.n_waves = e.n_waves; prm.grid = e.grid;
       memcpy(prm.unit_prefix, e.unit_prefix, sizeof(int32_t) * (prm.n_units + 1));
       memcpy(prm.pool_begin, e.pool_begin, sizeof(int64_t) * (e.grid + 1));
@@ -1218,7 +1250,8 @@ int64_t schedule_for(Params& prm, const ws_block_mask* mask, int sms) {
   const int64_t Tp = build_unit_prefix(prm, mask, prm.Lq, prm.cache_len, nullptr);
   build_schedule(prm, Tp, sms);
   victim->valid = true; victim->stamp = ++clock; victim->key = key;
-  victim->n_cache_tiles = prm.n_cache_tiles; victim->last_single = prm.last_single; victim->last_kv_tiles = prm.last_kv_tiles;
+  victim->n_cache_tiles = prm.n_cache_tiles; victim->n_tiles_a = prm.n_tiles_a; victim->len_a = prm.len_a;
+  victim->last_single = prm.last_single; victim->last_kv_tiles = prm.last_kv_tiles;
   victim->n_waves = prm.n_waves; victim->grid = prm.grid;
   memcpy(victim->unit_prefix, prm.unit_prefix, sizeof(int32_t) * (prm.n_units + 1));
   memcpy(victim->pool_begin, prm.pool_begin, sizeof(int64_t) * (prm.grid + 1));
@@ -1292,13 +1325,15 @@ namespace {
 int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const void* v_cache, int64_t capacity,
               int64_t cache_len, const void* k_new, const void* v_new, int32_t Ln, int32_t H, int32_t d, int32_t Lq,
               const ws_block_mask* mask, float softmax_scale, void* workspace, size_t workspace_bytes, ws_dtype dt,
-              void* stream_, int64_t tok_heads, const int8_t* k_exp = nullptr, const int8_t* v_exp = nullptr) {
+              void* stream_, int64_t tok_heads, const int8_t* k_exp = nullptr, const int8_t* v_exp = nullptr, int64_t ring_start = 0) {
   cudaStream_t stream = (cudaStream_t)stream_;
   const bool kv8 = k_exp != nullptr;  // the cache holds E4M3 codes with per-row exponents (ws_block_causal_attn_fp8kv)
   // ---- validation, descriptors and schedule first: nothing is launched on any error ----
   if (const int rc = wsi::attn_validate(out, lse, q, k_cache, v_cache, capacity, cache_len, k_new, v_new, Ln, H, d, Lq, mask,
                                         softmax_scale, workspace, workspace_bytes, dt))
     return rc;
+  if (ring_start < 0 || (ring_start > 0 && ring_start >= capacity)) return WS_ERR_OUT_OF_RANGE;
+  if (ring_start > 0x7fffffffLL - cache_len - kBlockN) return WS_ERR_UNSUPPORTED;  // TMA row coordinates are int32
   const int n_units = (Lq + kPairM - 1) / kPairM;
   const WsLayout L = ws_layout(Lq, H, d, cache_len + Ln, cache_len, Ln, dt, true);
   if (!get_encode_fn()) return wsi::cuda_fail(cudaErrorNotSupported);
@@ -1315,6 +1350,10 @@ int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const v
   const void* kn_b = f32 ? ws + L.stage_kn : k_new;
   const void* vn_b = f32 ? ws + L.stage_vn : v_new;
   const int64_t cap_b = f32 ? cache_len : capacity;
+  // a ring's window: the staged FP32 copy is linearised by the cast kernels, the BF16 cache is read in place as two runs
+  const CacheRuns runs = cache_runs(capacity, ring_start, cache_len);
+  const int64_t ring_b = f32 ? 0 : ring_start;
+  const int64_t map_rows = ring_b + cache_len < cap_b ? ring_b + cache_len : cap_b;  // rows past the window's end read as zero
 
   Params prm;
   memset(&prm, 0, sizeof(prm));
@@ -1329,9 +1368,9 @@ int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const v
   if (kv8 && cache_len > 0) {
     ok = ok && encode_map_u8(&prm.map_kc, kc_b, d, cache_len, H, cap_b) && encode_map_u8(&prm.map_vc, vc_b, d, cache_len, H, cap_b);
   } else {
-    ok = ok && (cache_len > 0 ? encode_map(&prm.map_kc, kc_b, d, cache_len, H, row_b, row_b * cap_b, kBlockN, 1)
+    ok = ok && (cache_len > 0 ? encode_map(&prm.map_kc, kc_b, d, map_rows, H, row_b, row_b * cap_b, kBlockN, 1)
                               : encode_map(&prm.map_kc, q_b, d, H, Lq, row_b, tok_b, 1, kBlockN));
-    ok = ok && (cache_len > 0 ? encode_map(&prm.map_vc, vc_b, d, cache_len, H, row_b, row_b * cap_b, kBlockN, 1)
+    ok = ok && (cache_len > 0 ? encode_map(&prm.map_vc, vc_b, d, map_rows, H, row_b, row_b * cap_b, kBlockN, 1)
                               : encode_map(&prm.map_vc, q_b, d, H, Lq, row_b, tok_b, 1, kBlockN));
   }
   if (!ok) return wsi::cuda_fail(cudaErrorInvalidValue);
@@ -1341,7 +1380,8 @@ int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const v
   prm.part_o = reinterpret_cast<float*>(ws + L.part_o);
   prm.part_ml = reinterpret_cast<float2*>(ws + L.part_ml);
   prm.cache_len = cache_len;
-  prm.capacity = capacity;
+  prm.capacity = f32 ? cache_len : capacity;
+  prm.ring_start = ring_b;
   prm.k_exp = k_exp;
   prm.v_exp = v_exp;
   prm.Lq = Lq; prm.H = H; prm.Ln = Ln; prm.n_blocks = mask->n_blocks; prm.n_units = n_units;
@@ -1359,20 +1399,28 @@ int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const v
   if (f32) {
     int launches = 0;
     cudaError_t ce = cudaSuccess;
-    auto cast = [&](const void* dstp, const void* srcp, int64_t planes, int64_t plane_elems, int64_t pitch) {
+    auto cast = [&](const void* dstp, int64_t dst_pitch, const void* srcp, int64_t planes, int64_t plane_elems, int64_t pitch) {
       const int64_t total = planes * plane_elems;
       if (total == 0 || ce != cudaSuccess) return;
       const int blocks = (int)((total + 255) / 256 < 4096 ? (total + 255) / 256 : 4096);
       ce = wsi::launch_pdl(cast_f32_to_bf16_kernel, dim3(blocks), dim3(256), 0, stream,
                            reinterpret_cast<__nv_bfloat16*>(const_cast<void*>(dstp)), reinterpret_cast<const float*>(srcp), planes,
-                           plane_elems, pitch);
+                           plane_elems, pitch, dst_pitch);
       if (ce == cudaSuccess) ++launches;
     };
-    cast(q_b, q, Lq, (int64_t)H * d, tok_heads * d);  // token by token: the staged copy is compact [Lq, H, d]
-    cast(kc_b, k_cache, H, cache_len * d, capacity * d);
-    cast(vc_b, v_cache, H, cache_len * d, capacity * d);
-    cast(kn_b, k_new, Ln, (int64_t)H * d, tok_heads * d);
-    cast(vn_b, v_new, Ln, (int64_t)H * d, tok_heads * d);
+    const int64_t hd = (int64_t)H * d;
+    cast(q_b, hd, q, Lq, hd, tok_heads * d);  // token by token: the staged copy is compact [Lq, H, d]
+    // the cache window in timeline order: run A (from ring_start), then run B (from physical row 0)
+    const float* kc_f = reinterpret_cast<const float*>(k_cache);
+    const float* vc_f = reinterpret_cast<const float*>(v_cache);
+    __nv_bfloat16* kc_s = reinterpret_cast<__nv_bfloat16*>(const_cast<void*>(kc_b));
+    __nv_bfloat16* vc_s = reinterpret_cast<__nv_bfloat16*>(const_cast<void*>(vc_b));
+    cast(kc_s, cache_len * d, kc_f + ring_start * d, H, runs.len_a * d, capacity * d);
+    cast(vc_s, cache_len * d, vc_f + ring_start * d, H, runs.len_a * d, capacity * d);
+    cast(kc_s + runs.len_a * d, cache_len * d, kc_f, H, runs.len_b * d, capacity * d);
+    cast(vc_s + runs.len_a * d, cache_len * d, vc_f, H, runs.len_b * d, capacity * d);
+    cast(kn_b, hd, k_new, Ln, hd, tok_heads * d);
+    cast(vn_b, hd, v_new, Ln, hd, tok_heads * d);
     if (launches) wsi::count_launch(launches);
     if (ce != cudaSuccess) return wsi::cuda_fail(ce);
   }
@@ -1404,6 +1452,17 @@ extern "C" __attribute__((visibility("default"))) int ws_block_causal_attn_seq_l
   return attn_impl(out_seq ? static_cast<char*>(out_seq) + off : nullptr, lse, shift(q_seq), k_cache, v_cache, capacity, cache_len,
                    shift(k_new_seq), shift(v_new_seq), Ln, H, d, Lq, mask, softmax_scale, workspace, workspace_bytes, dt, stream,
                    H_total);
+}
+
+// a3 on a ring (sliding-window) cache, SURVEY.md 8(f).4 / DESIGN.md R19: cache key j of the timeline is physical row
+// (ring_start + j) mod capacity.  The window is at most two physical runs of the cache tensor; each is tiled on its own.
+extern "C" __attribute__((visibility("default"))) int ws_block_causal_attn_ring(void* out, float* lse, const void* q, const void* k_cache, const void* v_cache,
+                                         int64_t capacity, int64_t ring_start, int64_t cache_len, const void* k_new, const void* v_new,
+                                         int32_t Ln, int32_t H, int32_t d, int32_t Lq, const ws_block_mask* mask, float softmax_scale,
+                                         void* workspace, size_t workspace_bytes, ws_dtype dt, void* stream) {
+  if (ring_start < 0 || ring_start >= (capacity > 0 ? capacity : 1)) return WS_ERR_OUT_OF_RANGE;
+  return attn_impl(out, lse, q, k_cache, v_cache, capacity, cache_len, k_new, v_new, Ln, H, d, Lq, mask, softmax_scale, workspace,
+                   workspace_bytes, dt, stream, H, nullptr, nullptr, ring_start);
 }
 
 // a3 on an FP8 cache: the cache holds E4M3 codes and one power-of-two exponent per (row, head), written by

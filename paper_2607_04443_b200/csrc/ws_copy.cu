@@ -180,6 +180,41 @@ extern "C" __attribute__((visibility("default"))) int ws_kv_cache_write(void* k_
   return launch_copy(srcs2, dsts2, 2, H, n_rows, dv, dv, (int64_t)H_src * dv, capacity * dv, dv, (cudaStream_t)stream);
 }
 
+// Ring (sliding-window) cache write, SURVEY.md 8(f).4 / DESIGN.md R19: session row write_pos + r goes to physical row
+// (write_pos + r) mod capacity.  At most two physical runs: one launch each (the second only when the slice wraps).
+extern "C" __attribute__((visibility("default"))) int ws_kv_cache_write_ring(void* k_cache, void* v_cache, int64_t capacity, int32_t H, int32_t d, const void* k_src,
+                                      const void* v_src, int32_t n_rows, int32_t H_src, int32_t head_begin, int64_t write_pos,
+                                      ws_dtype dt, void* stream) {
+  if (write_pos < 0 || capacity <= 0) return capacity <= 0 ? WS_ERR_INVALID_ARG : WS_ERR_OUT_OF_RANGE;
+  if (n_rows > capacity) return WS_ERR_OUT_OF_RANGE;  // a call never overwrites a row it has written itself
+  const int64_t phys = write_pos % capacity;
+  const int64_t n_a = n_rows < capacity - phys ? n_rows : capacity - phys, n_b = n_rows - n_a;
+  // both runs are checked before the first launch (the second run starts at physical row 0 with the slice's rows n_a ..)
+  if (const int rc = wsi::cache_write_validate(k_cache, v_cache, capacity, H, d, k_src, v_src, n_rows, H_src, head_begin, n_b > 0 ? 0 : phys, dt))
+    return rc;
+  if (n_rows == 0) return WS_OK;
+  const int64_t row_bytes = (int64_t)d * wsi::elem_bytes(dt), dv = row_bytes / 16;
+  int rc = WS_OK;
+  for (int run = 0; run < 2 && rc == WS_OK; ++run) {
+    const int64_t n = run ? n_b : n_a, dst_row = run ? 0 : phys, src_row = run ? n_a : 0;
+    if (n == 0) continue;
+    const void* srcs2[2] = {reinterpret_cast<const char*>(k_src) + (src_row * H_src + head_begin) * row_bytes,
+                            reinterpret_cast<const char*>(v_src) + (src_row * H_src + head_begin) * row_bytes};
+    void* dsts2[2] = {reinterpret_cast<char*>(k_cache) + dst_row * row_bytes, reinterpret_cast<char*>(v_cache) + dst_row * row_bytes};
+    rc = launch_copy(srcs2, dsts2, 2, H, n, dv, dv, (int64_t)H_src * dv, capacity * dv, dv, (cudaStream_t)stream);
+  }
+  return rc;
+}
+
+// The window after rows_written rows of the session (host only): cache_len = min(rows_written, capacity) valid rows, the
+// oldest of which sits in physical row ring_start.
+extern "C" __attribute__((visibility("default"))) int ws_ring_state(int64_t rows_written, int64_t capacity, int64_t* ring_start, int64_t* cache_len) {
+  if (rows_written < 0 || capacity <= 0 || !ring_start || !cache_len) return WS_ERR_INVALID_ARG;
+  *ring_start = rows_written < capacity ? 0 : rows_written % capacity;
+  *cache_len = rows_written < capacity ? rows_written : capacity;
+  return WS_OK;
+}
+
 extern "C" __attribute__((visibility("default"))) int ws_seq_to_head(void* dst, const void* src, int64_t n_tok, int32_t H, int32_t d, int32_t P, int32_t g0, int32_t G,
                               ws_dtype dt, void* stream) {
   return relayout(&dst, &src, 1, n_tok, H, d, P, g0, G, dt, stream, true);

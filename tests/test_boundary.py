@@ -122,6 +122,57 @@ def test_attention_rejects_bad_arguments(lib):
     assert call(qe=tuple(range(1, 131)), kv=tuple([576] * 130), Lq=130) == UNSUPPORTED  # > WS_MAX_MASK_BLOCKS
 
 
+def test_ring_entry_points_reject_bad_arguments_and_ring_state_is_host_only(lib):
+    """the ring cache write / attention check everything before CUDA is touched; ws_ring_state is pure
+    host logic and is compared with the rule of DESIGN.md R19 written out again here."""
+    i64 = ctypes.c_int64
+    for W in list(range(0, 40)) + [10 ** 12 + 3]:
+        for cap in (1, 7, 16):
+            a, b = i64(-5), i64(-5)
+            assert lib.ws_ring_state(W, cap, ctypes.byref(a), ctypes.byref(b)) == OK
+            assert (a.value, b.value) == ((0, W) if W < cap else (W % cap, cap))
+    a, b = i64(), i64()
+    assert lib.ws_ring_state(-1, 4, ctypes.byref(a), ctypes.byref(b)) == INVALID
+    assert lib.ws_ring_state(4, 0, ctypes.byref(a), ctypes.byref(b)) == INVALID
+    assert lib.ws_ring_state(4, 4, None, ctypes.byref(b)) == INVALID
+
+    w = lib.ws_kv_cache_write_ring
+    good = dict(kc=A, vc=B, cap=1024, H=4, d=128, ks=C, vs=D, n=64, Hs=8, hb=2, pos=1000, dt=0)
+
+    def wcall(**kw):
+        a = dict(good, **kw)
+        return w(P(a["kc"]), P(a["vc"]), a["cap"], a["H"], a["d"], P(a["ks"]), P(a["vs"]), a["n"], a["Hs"], a["hb"], a["pos"],
+                 a["dt"], None)
+
+    assert wcall(pos=-1) == RANGE
+    assert wcall(n=1025) == RANGE             # more rows than the ring holds
+    assert wcall(cap=0) == INVALID
+    assert wcall(hb=5) == INVALID
+    assert wcall(dt=7) == UNSUPPORTED
+    assert wcall(kc=A + 8) == ALIGN
+    assert wcall(ks=A + 4096) == OVERLAP
+    assert wcall(n=0) == OK                   # nothing launched
+    if not torch.cuda.is_available():
+        assert wcall() == CUDA                # a valid (wrapping) write reaches CUDA: no CPU fallback
+
+    f = lib.ws_block_causal_attn_ring
+    Mask = binding._BlockMask
+
+    def acall(cap=512, start=100, Tc=512, Ln=64, kv=(544, 576), q=B, d=128):
+        m = Mask(2, (ctypes.c_int32 * 2)(32, 64), (ctypes.c_int32 * 2)(*kv))
+        return f(P(A), None, P(q), P(C), P(D), cap, start, Tc, P(0x50000000), P(0x60000000), Ln, 2, d, 64, ctypes.byref(m), 0.1,
+                 P(0x70000000), 1 << 30, 0, None)
+
+    assert acall(start=-1) == RANGE
+    assert acall(start=512) == RANGE
+    assert acall(Tc=513) == RANGE
+    assert acall(kv=(544, 577)) == RANGE
+    assert acall(q=B + 8) == ALIGN
+    assert acall(d=96) == UNSUPPORTED
+    if not torch.cuda.is_available():
+        assert acall() == CUDA
+
+
 def test_unit_forward_host_checks_everything_before_enqueueing(lib):
     """ws_unit_forward_host runs every check of the calls it is made of (cache write, attention) up front, so a call
     that will fail enqueues no copy and forks no helper stream.  On this CPU-only box that is observable: every
