@@ -17,6 +17,9 @@
  *                           power-of-two scale per (row, head)): half the bytes of the full-history cache
  *   ws_kv_cache_write_ring / ws_block_causal_attn_ring / ws_ring_state   the cache as a sliding window over an
  *                           unbounded session: a ring that keeps the most recent `capacity` rows
+ *   ws_ulysses_push_seq_to_head / ws_block_causal_attn_push_out / ws_kv_slice_broadcast_write   the exchanges of a
+ *                           multi-GPU Ulysses performer group done as stores into peer memory (NVLink P2P) by the
+ *                           pack kernel, the attention epilogue and the cache-write kernel themselves
  *   ws_unit_forward_host   the same path for one unit fed from HOST buffers (end-to-end entry)
  *   ws_attn_schedule       host-only diagnostic: the attention work schedule for a given SM count
  *
@@ -69,6 +72,7 @@ typedef enum {
 
 /* Limits of this build. */
 #define WS_MAX_MASK_BLOCKS 128 /* n_blocks of a ws_block_mask */
+#define WS_MAX_PEERS 8         /* ranks of a Ulysses performer group (ws_ulysses_*, ws_block_causal_attn_push_out) */
 
 /* ------------------------------------------------------------------------------------------------
  * a1. KV cache write
@@ -248,6 +252,50 @@ int ws_block_causal_attn_ring(void* out, float* lse, const void* q, const void* 
                               int64_t ring_start, int64_t cache_len, const void* k_new, const void* v_new, int32_t Ln, int32_t H,
                               int32_t d, int32_t Lq, const ws_block_mask* mask, float softmax_scale, void* workspace,
                               size_t workspace_bytes, ws_dtype dt, void* stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * Ulysses exchange over peer memory ("denoising for the long latent video sequence is split
+ * across ranks with Ulysses all-to-all/gather communication.  Audio latents ... are generated without sequence sharding",
+ * :65 "Thinker broadcasts performer-compatible K/V slices", :73, :81).  Index maps: DESIGN.md reading R20.
+ *
+ *   P ranks (<= WS_MAX_PEERS), H heads in all, Hp = H / P per rank.  A unit's sequence is P * Ls sharded (video) tokens
+ *   followed by La unsharded (audio) tokens.  Rank r holds X_r [Ls + La, H, d]: its Ls video tokens, then the La audio
+ *   tokens (replicated on every rank).  Attention is head-parallel: rank g needs Y_g [P * Ls + La, Hp, d].
+ *
+ *   "Peer pointers" are device pointers valid in the CALLING process: local memory, or another GPU's memory mapped
+ *   through CUDA peer access / IPC / symmetric memory.  The kernels store through them directly (push model), so the
+ *   pack (a2), the unpack (a4) and the cache write (a1) ARE the transport: nothing is staged, no collective library
+ *   runs on the data path.  The calls are stream-ordered on the caller's stream and do not synchronise ranks: a
+ *   receiver must not read until every sender's call has completed (a barrier between the ranks' streams, e.g. one
+ *   torch.distributed barrier or a symmetric-memory signal per exchange), and a sender must not overwrite a buffer a
+ *   receiver is still reading.  On a single GPU all peers are local buffers and stream order is enough.
+ *
+ *   ws_ulysses_push_seq_to_head   exchange #1 (all-to-all) for up to 4 tensors (Q, K_new, V_new) in one call, run by rank `rank`:
+ *       Y_g[rank * Ls + t, c, :] = X[t, g * Hp + c, :]    for every peer g (stored through peer_dsts[i * P + g])
+ *       Y_rank[P * Ls + a, c, :] = X[Ls + a, rank * Hp + c, :]   (the audio rows are replicated: local)
+ *     peer_dsts : host array [n_tensors * P] of peer pointers to tensor i's Y_g;   srcs : host array [n_tensors] of X.
+ *   ws_block_causal_attn_push_out   a3 with exchange #2 fused into its epilogue, run by rank `rank` on its H (= Hp) heads:
+ *     q, k_new, v_new, caches, lse, mask, workspace exactly as ws_block_causal_attn with Lq = P * Ls + La; the output
+ *     row i of head c is stored to
+ *       Z_r[t, rank * H + c, :],      r = i / Ls, t = i % Ls          for i <  P * Ls   (all-to-all)
+ *       Z_r[Ls + (i - P * Ls), rank * H + c, :]  for EVERY r          for i >= P * Ls   (all-gather of the audio rows)
+ *     peer_outs : host array [P] of peer pointers to Z_r [Ls + La, P * H, d]; other heads of Z_r are not touched.
+ *   ws_kv_slice_broadcast_write   a1 on every rank by one kernel (the thinker's broadcast fused with the cache write):
+ *       cache_g[h, row_offset + i, :] = src[i, g * Hp + h, :]       peer_k_caches / peer_v_caches : host arrays [P]
+ *   Errors: as a2 / a3 / a1, plus UNSUPPORTED for P > WS_MAX_PEERS, INVALID_ARG for a NULL peer pointer or rank outside
+ *   [0, P), OUT_OF_RANGE if P * Ls > Lq, OVERLAP if two destinations (or a destination and a source) intersect.
+ * ---------------------------------------------------------------------------------------------- */
+int ws_ulysses_push_seq_to_head(void* const* peer_dsts, const void* const* srcs, int32_t n_tensors, int64_t Ls, int64_t La,
+                                int32_t H, int32_t d, int32_t P, int32_t rank, ws_dtype dt, void* stream);
+
+int ws_block_causal_attn_push_out(void* const* peer_outs, int32_t P, int32_t rank, int64_t Ls, float* lse, const void* q,
+                                  const void* k_cache, const void* v_cache, int64_t capacity, int64_t cache_len, const void* k_new,
+                                  const void* v_new, int32_t Ln, int32_t H, int32_t d, int32_t Lq, const ws_block_mask* mask,
+                                  float softmax_scale, void* workspace, size_t workspace_bytes, ws_dtype dt, void* stream);
+
+int ws_kv_slice_broadcast_write(void* const* peer_k_caches, void* const* peer_v_caches, int32_t P, int64_t capacity, int32_t Hp,
+                                int32_t d, const void* k_src, const void* v_src, int32_t n_rows, int64_t row_offset, ws_dtype dt,
+                                void* stream);
 
 /* ------------------------------------------------------------------------------------------------
  * a5. One unit end to end from HOST buffers ("receive the current K/V slice, update

@@ -11,6 +11,7 @@ from .binding import (  # noqa: F401
     block_causal_attn, block_causal_attn_workspace_bytes, block_causal_attn_seq_layout,
     kv_cache_write_fp8, block_causal_attn_fp8kv,
     kv_cache_write_ring, block_causal_attn_ring, ring_state,
+    ulysses_push_seq_to_head, block_causal_attn_push_out, kv_slice_broadcast_write,
     unit_forward_host, unit_forward_host_staging_bytes, kernel_launch_count, attn_schedule, EXPORTS,
     DTYPE_BF16, DTYPE_F32,
 )

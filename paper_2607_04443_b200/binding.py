@@ -24,6 +24,7 @@ EXPORTS = (
     "ws_block_causal_attn", "ws_block_causal_attn_seq_layout", "ws_unit_forward_host_staging_bytes", "ws_unit_forward_host", "ws_status_string",
     "ws_version", "ws_last_cuda_error", "ws_kernel_launch_count", "ws_attn_schedule", "ws_kv_cache_write_fp8", "ws_block_causal_attn_fp8kv",
     "ws_kv_cache_write_ring", "ws_ring_state", "ws_block_causal_attn_ring",
+    "ws_ulysses_push_seq_to_head", "ws_block_causal_attn_push_out", "ws_kv_slice_broadcast_write",
 )
 
 
@@ -91,6 +92,13 @@ def load():
     lib.ws_block_causal_attn_ring.argtypes = [vp, vp, vp, vp, vp, i64, i64, i64, vp, vp, i32, i32, i32, i32,
                                               ctypes.POINTER(_BlockMask), f32, vp, sz, ctypes.c_int, vp]
     lib.ws_block_causal_attn_ring.restype = ctypes.c_int
+    lib.ws_ulysses_push_seq_to_head.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(vp), i32, i64, i64, i32, i32, i32, i32, ctypes.c_int, vp]
+    lib.ws_ulysses_push_seq_to_head.restype = ctypes.c_int
+    lib.ws_block_causal_attn_push_out.argtypes = [ctypes.POINTER(vp), i32, i32, i64, vp, vp, vp, vp, i64, i64, vp, vp, i32, i32, i32, i32,
+                                                  ctypes.POINTER(_BlockMask), f32, vp, sz, ctypes.c_int, vp]
+    lib.ws_block_causal_attn_push_out.restype = ctypes.c_int
+    lib.ws_kv_slice_broadcast_write.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(vp), i32, i64, i32, i32, vp, vp, i32, i64, ctypes.c_int, vp]
+    lib.ws_kv_slice_broadcast_write.restype = ctypes.c_int
     lib.ws_status_string.argtypes = [ctypes.c_int]
     lib.ws_status_string.restype = ctypes.c_char_p
     for fn in (lib.ws_version, lib.ws_last_cuda_error, lib.ws_kernel_launch_count):
@@ -295,6 +303,89 @@ def block_causal_attn_ring(out, q, k_cache, v_cache, ring_start: int, cache_len:
                                           _p(k_new), _p(v_new), Ln, H, d, Lq, ctypes.byref(mask), float(softmax_scale), _p(workspace),
                                           workspace.numel() * workspace.element_size(), _dt(q), _stream(stream))
     _ok(rc, "ws_block_causal_attn_ring")
+
+
+def _ptr_array(tensors):
+    return (ctypes.c_void_p * len(tensors))(*[t.data_ptr() for t in tensors])
+
+
+def ulysses_push_seq_to_head(peer_dsts, srcs, Ls: int, rank: int, stream=None):
+    """Exchange #1 of a Ulysses group, run by rank `rank` (ws.h ws_ulysses_push_seq_to_head).  srcs: this rank's tensors
+    X [Ls + La, H, d] (up to 4: Q, K_new, V_new); peer_dsts[i][g]: tensor i's Y_g [P * Ls + La, H / P, d] on peer g
+    (a tensor in this process's address space: local, or peer-mapped)."""
+    srcs = list(srcs)
+    P = len(peer_dsts[0])
+    flat = [t for row in peer_dsts for t in row]
+    _dev(*srcs, *flat)
+    n, H, d = srcs[0].shape
+    La = n - Ls
+    for x in srcs:
+        if tuple(x.shape) != (n, H, d) or x.dtype != srcs[0].dtype:
+            raise ValueError("ws_ulysses_push_seq_to_head: sources must share shape and dtype")
+    for row in peer_dsts:
+        if len(row) != P:
+            raise ValueError("ws_ulysses_push_seq_to_head: every tensor needs one destination per peer")
+        for y in row:
+            if y.dtype != srcs[0].dtype or (H % P == 0 and tuple(y.shape) != (P * Ls + La, H // P, d)):
+                raise ValueError("ws_ulysses_push_seq_to_head: destinations must be [P * Ls + La, H / P, d]")
+    rc = load().ws_ulysses_push_seq_to_head(_ptr_array(flat), _ptr_array(srcs), len(srcs), int(Ls), int(La), H, d, P, int(rank),
+                                            _dt(srcs[0]), _stream(stream))
+    _ok(rc, "ws_ulysses_push_seq_to_head")
+
+
+def block_causal_attn_push_out(peer_outs, rank: int, Ls: int, q, k_cache, v_cache, cache_len: int, k_new, v_new,
+                               q_block_end: Sequence[int], kv_visible: Sequence[int], softmax_scale: float, workspace, lse=None,
+                               stream=None):
+    """Attention of rank `rank` on its heads with exchange #2 fused into the epilogue (ws.h ws_block_causal_attn_push_out).
+    peer_outs[r]: peer r's token-major output Z_r [Ls + La, P * H, d]; q [P * Ls + La, H, d]."""
+    peer_outs = list(peer_outs)
+    _dev(*peer_outs, q, k_cache, v_cache, k_new, v_new, workspace, lse)
+    P = len(peer_outs)
+    Lq, H, d = q.shape
+    capacity = k_cache.shape[1]
+    Ln = 0 if k_new is None else k_new.shape[0]
+    La = Lq - P * Ls
+    for z in peer_outs:
+        if z.dtype != q.dtype or tuple(z.shape) != (Ls + La, P * H, d):
+            raise ValueError("ws_block_causal_attn_push_out: peer outputs must be [Ls + La, P * H, d]")
+    if tuple(k_cache.shape) != (H, capacity, d) or v_cache.shape != k_cache.shape:
+        raise ValueError("ws_block_causal_attn_push_out: cache must be [H, capacity, d]")
+    if k_new is not None and (tuple(k_new.shape) != (Ln, H, d) or v_new is None or v_new.shape != k_new.shape):
+        raise ValueError("ws_block_causal_attn_push_out: k_new/v_new must be [Ln, H, d]")
+    for t in (k_cache, v_cache, k_new, v_new):
+        if t is not None and t.dtype != q.dtype:
+            raise TypeError("ws_block_causal_attn_push_out: dtype mismatch")
+    if lse is not None and (lse.dtype != torch.float32 or tuple(lse.shape) != (H, Lq)):
+        raise ValueError("ws_block_causal_attn_push_out: lse must be float32 [H, Lq]")
+    n = len(q_block_end)
+    if len(kv_visible) != n:
+        raise ValueError("ws_block_causal_attn_push_out: mask arrays differ in length")
+    qe = (ctypes.c_int32 * n)(*[int(x) for x in q_block_end])
+    kv = (ctypes.c_int32 * n)(*[int(x) for x in kv_visible])
+    mask = _BlockMask(n, qe, kv)
+    rc = load().ws_block_causal_attn_push_out(_ptr_array(peer_outs), P, int(rank), int(Ls), _p(lse), _p(q), _p(k_cache), _p(v_cache),
+                                              capacity, int(cache_len), _p(k_new), _p(v_new), Ln, H, d, Lq, ctypes.byref(mask),
+                                              float(softmax_scale), _p(workspace), workspace.numel() * workspace.element_size(),
+                                              _dt(q), _stream(stream))
+    _ok(rc, "ws_block_causal_attn_push_out")
+
+
+def kv_slice_broadcast_write(peer_k_caches, peer_v_caches, k_src, v_src, row_offset: int = 0, stream=None):
+    """The thinker's slice [n_rows, P * Hp, d] written into every rank's cache [Hp, capacity, d] by one kernel
+    (ws.h ws_kv_slice_broadcast_write)."""
+    peer_k_caches, peer_v_caches = list(peer_k_caches), list(peer_v_caches)
+    _dev(*peer_k_caches, *peer_v_caches, k_src, v_src)
+    P = len(peer_k_caches)
+    Hp, capacity, d = peer_k_caches[0].shape
+    n_rows = k_src.shape[0]
+    if len(peer_v_caches) != P or tuple(k_src.shape) != (n_rows, P * Hp, d) or v_src.shape != k_src.shape:
+        raise ValueError("ws_kv_slice_broadcast_write: shape mismatch")
+    for c in peer_k_caches + peer_v_caches:
+        if tuple(c.shape) != (Hp, capacity, d) or c.dtype != k_src.dtype:
+            raise ValueError("ws_kv_slice_broadcast_write: every cache must be [Hp, capacity, d] of the slice's dtype")
+    rc = load().ws_kv_slice_broadcast_write(_ptr_array(peer_k_caches), _ptr_array(peer_v_caches), P, capacity, Hp, d, _p(k_src),
+                                            _p(v_src), n_rows, int(row_offset), _dt(k_src), _stream(stream))
+    _ok(rc, "ws_kv_slice_broadcast_write")
 
 
 def kv_cache_write_fp8(k_cache8, v_cache8, k_exp, v_exp, k_src, v_src, head_begin: int = 0, row_offset: int = 0, stream=None):

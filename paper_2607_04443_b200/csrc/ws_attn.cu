@@ -83,7 +83,12 @@ constexpr int kPReadyArrivals = WS_WARP_ARRIVE ? 4 : 128;  // arrivals per P-chu
 
 struct alignas(64) Params {
   CUtensorMap map_q, map_kn, map_vn, map_kc, map_vc;
-  void* out;
+  // Output rows.  Plain call: n_peers == 1, out_peer[0] = the [Lq, *, d] output.  ws_block_causal_attn_push_out (exchange #2 of
+  // the Ulysses group fused into the epilogue): row i < n_peers * peer_rows goes to peer i / peer_rows, local row i % peer_rows;
+  // the unsharded rows behind them go to EVERY peer at local row peer_rows + (i - n_peers * peer_rows).  The pointers
+  // already carry the offset of this rank's first head.
+  void* out_peer[WS_MAX_PEERS];
+  int32_t n_peers, peer_rows;
   float* lse;
   float* part_o;   // [records][d/4][128][4]
   float2* part_ml; // [records][128] (m * scale * log2e, l)
@@ -127,6 +132,31 @@ __device__ __forceinline__ int block_of_row(const Params& p, int row) {
     if (row < p.q_block_end[mid]) hi = mid; else lo = mid + 1;
   }
   return lo;
+}
+
+// Where output row `row` goes: destinations out_peer[peer0 .. peer0 + n_dst), each at element offset elem_off (to which the
+// caller adds head * D + column).
+struct RowDst {
+  int peer0, n_dst;
+  int64_t elem_off;
+};
+__device__ __forceinline__ RowDst row_dst(const Params& p, int row) {
+  RowDst r;
+  r.peer0 = 0;
+  r.n_dst = 1;
+  int64_t local = row;
+  if (p.n_peers > 1) {
+    const int sharded = p.n_peers * p.peer_rows;
+    if (row < sharded) {
+      r.peer0 = row / p.peer_rows;
+      local = row - r.peer0 * p.peer_rows;
+    } else {
+      r.n_dst = p.n_peers;
+      local = p.peer_rows + (row - sharded);
+    }
+  }
+  r.elem_off = local * p.out_pitch;
+  return r;
 }
 
 __device__ __forceinline__ int unit_of_iter(const Params& s, int rem) {
@@ -604,6 +634,7 @@ __global__ void __launch_bounds__(KV8 ? kThreads8 : kThreads, 1) attn_fwd_kernel
 
     // final rows: O / l in the output dtype, LSE
     auto store_row = [&](int head, int row, float inv, uint32_t t_src, auto&& transform) {
+      const RowDst rd = row_dst(p, row);
 #pragma unroll
       for (int ch = 0; ch < D / 32; ++ch) {
         uint32_t o[32];
@@ -611,22 +642,31 @@ __global__ void __launch_bounds__(KV8 ? kThreads8 : kThreads, 1) attn_fwd_kernel
         ptx::tc_wait_ld();
         transform(ch, o);
         if (row < p.Lq) {
+          const int64_t off = rd.elem_off + (int64_t)head * D + ch * 32;
           if constexpr (OUT_F32) {
-            float4* dst = reinterpret_cast<float4*>(reinterpret_cast<float*>(p.out) + ((int64_t)row * p.out_pitch + (int64_t)head * D) + ch * 32);
+            float4 v[8];
 #pragma unroll
             for (int c = 0; c < 8; ++c)
-              dst[c] = make_float4(__uint_as_float(o[4 * c]) * inv, __uint_as_float(o[4 * c + 1]) * inv,
-                                   __uint_as_float(o[4 * c + 2]) * inv, __uint_as_float(o[4 * c + 3]) * inv);
+              v[c] = make_float4(__uint_as_float(o[4 * c]) * inv, __uint_as_float(o[4 * c + 1]) * inv,
+                                 __uint_as_float(o[4 * c + 2]) * inv, __uint_as_float(o[4 * c + 3]) * inv);
+            for (int k = 0; k < rd.n_dst; ++k) {
+              float4* dst = reinterpret_cast<float4*>(reinterpret_cast<float*>(p.out_peer[rd.peer0 + k]) + off);
+#pragma unroll
+              for (int c = 0; c < 8; ++c) dst[c] = v[c];
+            }
           } else {
-            uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<__nv_bfloat16*>(p.out) + ((int64_t)row * p.out_pitch + (int64_t)head * D) + ch * 32);
+            uint4 v[4];
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
-              uint4 v;
-              v.x = ptx::pack_bf16(__uint_as_float(o[8 * c]) * inv, __uint_as_float(o[8 * c + 1]) * inv);
-              v.y = ptx::pack_bf16(__uint_as_float(o[8 * c + 2]) * inv, __uint_as_float(o[8 * c + 3]) * inv);
-              v.z = ptx::pack_bf16(__uint_as_float(o[8 * c + 4]) * inv, __uint_as_float(o[8 * c + 5]) * inv);
-              v.w = ptx::pack_bf16(__uint_as_float(o[8 * c + 6]) * inv, __uint_as_float(o[8 * c + 7]) * inv);
-              dst[c] = v;
+              v[c].x = ptx::pack_bf16(__uint_as_float(o[8 * c]) * inv, __uint_as_float(o[8 * c + 1]) * inv);
+              v[c].y = ptx::pack_bf16(__uint_as_float(o[8 * c + 2]) * inv, __uint_as_float(o[8 * c + 3]) * inv);
+              v[c].z = ptx::pack_bf16(__uint_as_float(o[8 * c + 4]) * inv, __uint_as_float(o[8 * c + 5]) * inv);
+              v[c].w = ptx::pack_bf16(__uint_as_float(o[8 * c + 6]) * inv, __uint_as_float(o[8 * c + 7]) * inv);
+            }
+            for (int k = 0; k < rd.n_dst; ++k) {
+              uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<__nv_bfloat16*>(p.out_peer[rd.peer0 + k]) + off);
+#pragma unroll
+              for (int c = 0; c < 4; ++c) dst[c] = v[c];
             }
           }
         }
@@ -643,9 +683,12 @@ __global__ void __launch_bounds__(KV8 ? kThreads8 : kThreads, 1) attn_fwd_kernel
         if (row_valid && !(sp.single && tile == 1)) {
           if (p.lse != nullptr) p.lse[(int64_t)g.head * p.Lq + row] = -INFINITY;
           constexpr int kRowVecs = D * (OUT_F32 ? 4 : 2) / 16;
-          uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<char*>(p.out) + ((int64_t)row * p.out_pitch + (int64_t)g.head * D) * (OUT_F32 ? 4 : 2));
+          const RowDst rd = row_dst(p, row);
+          for (int k = 0; k < rd.n_dst; ++k) {
+            uint4* dst = reinterpret_cast<uint4*>(reinterpret_cast<char*>(p.out_peer[rd.peer0 + k]) + (rd.elem_off + (int64_t)g.head * D) * (OUT_F32 ? 4 : 2));
 #pragma unroll
-          for (int c = 0; c < kRowVecs; ++c) dst[c] = make_uint4(0u, 0u, 0u, 0u);
+            for (int c = 0; c < kRowVecs; ++c) dst[c] = make_uint4(0u, 0u, 0u, 0u);
+          }
         }
         continue;
       }
@@ -882,14 +925,17 @@ __global__ void __launch_bounds__(kPairM) attn_combine_kernel(const __grid_const
       acc = make_float4(0.f, 0.f, 0.f, 0.f);
     }
   }
-  const int64_t o_off = ((int64_t)row * p.out_pitch + (int64_t)head * D) + q4 * 4;
-  if constexpr (OUT_F32) {
-    *reinterpret_cast<float4*>(reinterpret_cast<float*>(p.out) + o_off) = acc;
-  } else {
-    uint2 v;
-    v.x = ptx::pack_bf16(acc.x, acc.y);
-    v.y = ptx::pack_bf16(acc.z, acc.w);
-    *reinterpret_cast<uint2*>(reinterpret_cast<__nv_bfloat16*>(p.out) + o_off) = v;
+  const RowDst rd = row_dst(p, row);
+  const int64_t o_off = rd.elem_off + (int64_t)head * D + q4 * 4;
+  for (int k = 0; k < rd.n_dst; ++k) {
+    if constexpr (OUT_F32) {
+      *reinterpret_cast<float4*>(reinterpret_cast<float*>(p.out_peer[rd.peer0 + k]) + o_off) = acc;
+    } else {
+      uint2 v;
+      v.x = ptx::pack_bf16(acc.x, acc.y);
+      v.y = ptx::pack_bf16(acc.z, acc.w);
+      *reinterpret_cast<uint2*>(reinterpret_cast<__nv_bfloat16*>(p.out_peer[rd.peer0 + k]) + o_off) = v;
+    }
   }
   if (q4 == 0 && p.lse != nullptr) p.lse[(int64_t)head * p.Lq + row] = lse;
 }
@@ -1325,7 +1371,8 @@ namespace {
 int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const void* v_cache, int64_t capacity,
               int64_t cache_len, const void* k_new, const void* v_new, int32_t Ln, int32_t H, int32_t d, int32_t Lq,
               const ws_block_mask* mask, float softmax_scale, void* workspace, size_t workspace_bytes, ws_dtype dt,
-              void* stream_, int64_t tok_heads, const int8_t* k_exp = nullptr, const int8_t* v_exp = nullptr, int64_t ring_start = 0) {
+              void* stream_, int64_t tok_heads, const int8_t* k_exp = nullptr, const int8_t* v_exp = nullptr, int64_t ring_start = 0,
+              void* const* peer_outs = nullptr, int32_t n_peers = 1, int64_t peer_rows = 0) {
   cudaStream_t stream = (cudaStream_t)stream_;
   const bool kv8 = k_exp != nullptr;  // the cache holds E4M3 codes with per-row exponents (ws_block_causal_attn_fp8kv)
   // ---- validation, descriptors and schedule first: nothing is launched on any error ----
@@ -1374,8 +1421,16 @@ int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const v
                               : encode_map(&prm.map_vc, q_b, d, H, Lq, row_b, tok_b, 1, kBlockN));
   }
   if (!ok) return wsi::cuda_fail(cudaErrorInvalidValue);
-  prm.out = out;
-  prm.out_pitch = tok_heads * d;
+  if (peer_outs) {  // ws_block_causal_attn_push_out: `out` is peer 0's pointer (validated like a plain output)
+    for (int r = 0; r < n_peers; ++r) prm.out_peer[r] = peer_outs[r];
+    prm.n_peers = n_peers;
+    prm.peer_rows = (int32_t)peer_rows;
+  } else {
+    prm.out_peer[0] = out;
+    prm.n_peers = 1;
+    prm.peer_rows = 0x7fffffff;
+  }
+  prm.out_pitch = (peer_outs ? (int64_t)n_peers * H : tok_heads) * d;  // a peer's output rows hold the heads of all ranks
   prm.lse = lse;
   prm.part_o = reinterpret_cast<float*>(ws + L.part_o);
   prm.part_ml = reinterpret_cast<float2*>(ws + L.part_ml);
@@ -1452,6 +1507,35 @@ extern "C" __attribute__((visibility("default"))) int ws_block_causal_attn_seq_l
   return attn_impl(out_seq ? static_cast<char*>(out_seq) + off : nullptr, lse, shift(q_seq), k_cache, v_cache, capacity, cache_len,
                    shift(k_new_seq), shift(v_new_seq), Ln, H, d, Lq, mask, softmax_scale, workspace, workspace_bytes, dt, stream,
                    H_total);
+}
+
+// a3 with exchange #2 of the Ulysses group fused into its epilogue ("Ulysses all-to-all/gather
+// communication", :73; R20).  This rank (index `rank` of P) computes its H heads over the whole sequence
+// (P * Ls sharded rows, then Lq - P * Ls unsharded rows) and the softmax warps store every finished row straight into
+// the token-major [Ls + La, P * H, d] output of the peer that owns the row -- peer i / Ls for a sharded row i, EVERY peer
+// for an unsharded row (the all-gather) -- through peer-mapped pointers: the all-to-all is the epilogue's store, nothing is
+// staged and nothing is sent twice.
+extern "C" __attribute__((visibility("default"))) int ws_block_causal_attn_push_out(void* const* peer_outs, int32_t P, int32_t rank, int64_t Ls, float* lse, const void* q,
+                                             const void* k_cache, const void* v_cache, int64_t capacity, int64_t cache_len,
+                                             const void* k_new, const void* v_new, int32_t Ln, int32_t H, int32_t d, int32_t Lq,
+                                             const ws_block_mask* mask, float softmax_scale, void* workspace, size_t workspace_bytes,
+                                             ws_dtype dt, void* stream) {
+  if (dt != WS_DTYPE_BF16 && dt != WS_DTYPE_F32) return WS_ERR_UNSUPPORTED;
+  if (!peer_outs || P <= 0 || rank < 0 || rank >= P || Ls <= 0 || H <= 0 || d <= 0 || Lq <= 0) return WS_ERR_INVALID_ARG;
+  if (P > WS_MAX_PEERS) return WS_ERR_UNSUPPORTED;
+  if ((int64_t)P * Ls > Lq) return WS_ERR_OUT_OF_RANGE;
+  const int64_t off = (int64_t)rank * H * d * wsi::elem_bytes(dt);  // this rank's first head inside a [*, P * H, d] token row
+  void* shifted[WS_MAX_PEERS];
+  const size_t peer_bytes = (size_t)(Ls + (Lq - (int64_t)P * Ls)) * P * H * d * wsi::elem_bytes(dt);
+  for (int r = 0; r < P; ++r) {
+    if (!peer_outs[r]) return WS_ERR_INVALID_ARG;
+    if (!wsi::aligned16(peer_outs[r])) return WS_ERR_ALIGNMENT;
+    for (int j = 0; j < r; ++j)
+      if (wsi::ranges_overlap(peer_outs[r], peer_bytes, peer_outs[j], peer_bytes)) return WS_ERR_OVERLAP;
+    shifted[r] = static_cast<char*>(peer_outs[r]) + off;
+  }
+  return attn_impl(shifted[0], lse, q, k_cache, v_cache, capacity, cache_len, k_new, v_new, Ln, H, d, Lq, mask, softmax_scale, workspace,
+                   workspace_bytes, dt, stream, H, nullptr, nullptr, 0, shifted, P, Ls);
 }
 
 // a3 on a ring (sliding-window) cache, SURVEY.md 8(f).4 / DESIGN.md R19: cache key j of the timeline is physical row

@@ -19,10 +19,11 @@ namespace {
 constexpr int kThreads = 256;
 constexpr int kUnroll = 2;  // 16-byte vectors per thread
 
-constexpr int kMaxTensors = 4;  // tensors moved by one launch (blockIdx.z)
+constexpr int kMaxTensors = 4;   // tensors of one *_multi call (ws.h)
+constexpr int kMaxEntries = 16;  // (source, destination) pairs moved by one launch (blockIdx.z): tensors x peers
 struct CopyPtrs {
-  const uint4* src[kMaxTensors];
-  uint4* dst[kMaxTensors];
+  const uint4* src[kMaxEntries];
+  uint4* dst[kMaxEntries];
 };
 
 struct CopyPlan {
@@ -74,7 +75,7 @@ __global__ void __launch_bounds__(kThreads) strided_copy16_kernel(const __grid_c
 int launch_copy(const void* const* srcs, void* const* dsts, int n_tensors, int64_t A, int64_t B, int64_t dv, int64_t src_a,
                 int64_t src_b, int64_t dst_a, int64_t dst_b, cudaStream_t stream) {
   if (A == 0 || B == 0 || dv == 0 || n_tensors == 0) return WS_OK;
-  if (A > 65535 || dv > (1 << 20) || n_tensors > kMaxTensors) return WS_ERR_UNSUPPORTED;
+  if (A > 65535 || dv > (1 << 20) || n_tensors > kMaxEntries) return WS_ERR_UNSUPPORTED;
   const int64_t max_b = ((int64_t)1 << 30) / dv;
   int launches = 0;
   for (int64_t b0 = 0; b0 < B; b0 += max_b) {
@@ -204,6 +205,92 @@ extern "C" __attribute__((visibility("default"))) int ws_kv_cache_write_ring(voi
     rc = launch_copy(srcs2, dsts2, 2, H, n, dv, dv, (int64_t)H_src * dv, capacity * dv, dv, (cudaStream_t)stream);
   }
   return rc;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// Ulysses exchange over peer memory.  Push model: the sender's copy kernel stores
+// straight into the receivers' buffers through peer-mapped pointers (NVLink / NVSwitch P2P stores; on one GPU the "peers"
+// are local buffers), in the layout the attention kernel reads -- the pack (a2) and the transport are one kernel and
+// nothing is staged.  blockIdx.z walks the (tensor, peer) pairs.
+// ---------------------------------------------------------------------------------------------------------------------
+extern "C" __attribute__((visibility("default"))) int ws_ulysses_push_seq_to_head(void* const* peer_dsts, const void* const* srcs, int32_t n_tensors, int64_t Ls,
+                                           int64_t La, int32_t H, int32_t d, int32_t P, int32_t rank, ws_dtype dt, void* stream) {
+  const int es = wsi::elem_bytes(dt);
+  if (es == 0) return WS_ERR_UNSUPPORTED;
+  if (!peer_dsts || !srcs || n_tensors < 0 || Ls < 0 || La < 0 || H <= 0 || d <= 0 || P <= 0 || H % P != 0 || rank < 0 || rank >= P)
+    return WS_ERR_INVALID_ARG;
+  if (n_tensors > kMaxTensors || P > WS_MAX_PEERS) return WS_ERR_UNSUPPORTED;
+  if (((int64_t)d * es) % 16 != 0) return WS_ERR_ALIGNMENT;
+  const int32_t Hp = H / P;
+  const int64_t chunk_bytes = (int64_t)Hp * d * es, dv = chunk_bytes / 16, tok_b = (int64_t)H * d * es / 16;
+  const size_t src_bytes = (size_t)(Ls + La) * H * d * es, dst_bytes = (size_t)(P * Ls + La) * chunk_bytes;
+  for (int i = 0; i < n_tensors; ++i) {
+    if (!srcs[i]) return WS_ERR_INVALID_ARG;
+    if (!wsi::aligned16(srcs[i])) return WS_ERR_ALIGNMENT;
+    for (int g = 0; g < P; ++g) {
+      if (!peer_dsts[i * P + g]) return WS_ERR_INVALID_ARG;
+      if (!wsi::aligned16(peer_dsts[i * P + g])) return WS_ERR_ALIGNMENT;
+    }
+  }
+  // unified virtual addressing: a peer-mapped range and a local range intersect only if they are the same memory
+  for (int i = 0; i < n_tensors * P; ++i) {
+    for (int j = 0; j < n_tensors; ++j)
+      if (wsi::ranges_overlap(peer_dsts[i], dst_bytes, srcs[j], src_bytes)) return WS_ERR_OVERLAP;
+    for (int j = 0; j < i; ++j)
+      if (wsi::ranges_overlap(peer_dsts[i], dst_bytes, peer_dsts[j], dst_bytes)) return WS_ERR_OVERLAP;
+  }
+  // sharded (video) rows: Y_g[rank * Ls + t, c, :] = X[t, g * Hp + c, :] on every peer g
+  const void* s2[kMaxEntries];
+  void* d2[kMaxEntries];
+  int n = 0, rc = WS_OK;
+  for (int i = 0; i < n_tensors && rc == WS_OK; ++i)
+    for (int g = 0; g < P && rc == WS_OK; ++g) {
+      s2[n] = reinterpret_cast<const char*>(srcs[i]) + (int64_t)g * chunk_bytes;
+      d2[n] = reinterpret_cast<char*>(peer_dsts[i * P + g]) + (int64_t)rank * Ls * chunk_bytes;
+      if (++n == kMaxEntries || (i == n_tensors - 1 && g == P - 1)) {
+        rc = launch_copy(s2, d2, n, 1, Ls, dv, 0, tok_b, 0, dv, (cudaStream_t)stream);
+        n = 0;
+      }
+    }
+  // unsharded (audio) rows are replicated on every rank: the rank's own heads are a local relayout
+  for (int i = 0; i < n_tensors; ++i) {
+    s2[i] = reinterpret_cast<const char*>(srcs[i]) + (Ls * H + (int64_t)rank * Hp) * d * es;
+    d2[i] = reinterpret_cast<char*>(peer_dsts[i * P + rank]) + (int64_t)P * Ls * chunk_bytes;
+  }
+  if (rc == WS_OK) rc = launch_copy(s2, d2, n_tensors, 1, La, dv, 0, tok_b, 0, dv, (cudaStream_t)stream);
+  return rc;
+}
+
+// The thinker's K/V slice [n_rows, P * Hp, d] written into every performer rank's cache [Hp, capacity, d] by ONE kernel
+// (broadcast fused with a1): the slice is read once and each rank's head range is stored through that rank's peer pointer.
+extern "C" __attribute__((visibility("default"))) int ws_kv_slice_broadcast_write(void* const* peer_k_caches, void* const* peer_v_caches, int32_t P, int64_t capacity,
+                                           int32_t Hp, int32_t d, const void* k_src, const void* v_src, int32_t n_rows,
+                                           int64_t row_offset, ws_dtype dt, void* stream) {
+  if (!peer_k_caches || !peer_v_caches || P <= 0 || Hp <= 0) return WS_ERR_INVALID_ARG;
+  if (P > WS_MAX_PEERS) return WS_ERR_UNSUPPORTED;
+  if ((int64_t)P * Hp > 0x7fffffff) return WS_ERR_INVALID_ARG;
+  for (int g = 0; g < P; ++g)
+    if (const int rc = wsi::cache_write_validate(peer_k_caches[g], peer_v_caches[g], capacity, Hp, d, k_src, v_src, n_rows, P * Hp, g * Hp,
+                                                 row_offset, dt))
+      return rc;
+  const int64_t row_bytes = (int64_t)d * wsi::elem_bytes(dt), dv = row_bytes / 16;
+  const size_t cache_bytes = (size_t)Hp * capacity * row_bytes;
+  for (int g = 0; g < P; ++g)  // two ranks' caches must not be the same memory
+    for (int j = 0; j < g; ++j)
+      if (wsi::ranges_overlap(peer_k_caches[g], cache_bytes, peer_k_caches[j], cache_bytes) || wsi::ranges_overlap(peer_v_caches[g], cache_bytes, peer_v_caches[j], cache_bytes) ||
+          wsi::ranges_overlap(peer_k_caches[g], cache_bytes, peer_v_caches[j], cache_bytes) || wsi::ranges_overlap(peer_v_caches[g], cache_bytes, peer_k_caches[j], cache_bytes))
+        return WS_ERR_OVERLAP;
+  if (n_rows == 0) return WS_OK;
+  const void* s2[kMaxEntries];
+  void* d2[kMaxEntries];
+  for (int g = 0; g < P; ++g) {
+    s2[2 * g] = reinterpret_cast<const char*>(k_src) + (int64_t)g * Hp * row_bytes;
+    s2[2 * g + 1] = reinterpret_cast<const char*>(v_src) + (int64_t)g * Hp * row_bytes;
+    d2[2 * g] = reinterpret_cast<char*>(peer_k_caches[g]) + row_offset * row_bytes;
+    d2[2 * g + 1] = reinterpret_cast<char*>(peer_v_caches[g]) + row_offset * row_bytes;
+  }
+  static_assert(2 * WS_MAX_PEERS <= kMaxEntries, "one launch holds K and V of every peer");
+  return launch_copy(s2, d2, 2 * P, Hp, n_rows, dv, dv, (int64_t)P * Hp * dv, capacity * dv, dv, (cudaStream_t)stream);
 }
 
 // The window after rows_written rows of the session (host only): cache_len = min(rows_written, capacity) valid rows, the

@@ -173,6 +173,64 @@ def test_ring_entry_points_reject_bad_arguments_and_ring_state_is_host_only(lib)
         assert acall() == CUDA
 
 
+def test_ulysses_exchange_entry_points_reject_bad_arguments(lib):
+    """every argument error of the peer-memory exchange calls comes back before CUDA is touched."""
+    vp = ctypes.c_void_p
+
+    def arr(*ptrs):
+        return (vp * len(ptrs))(*ptrs)
+
+    push = lib.ws_ulysses_push_seq_to_head
+
+    def pcall(dsts=(A, B), srcs=(C,), n=1, Ls=16, La=4, H=8, d=64, Pn=2, rank=0, dt=0):
+        return push(arr(*dsts), arr(*srcs), n, Ls, La, H, d, Pn, rank, dt, None)
+
+    assert pcall(rank=2) == INVALID
+    assert pcall(rank=-1) == INVALID
+    assert pcall(H=7) == INVALID                       # H % P != 0
+    assert pcall(dsts=(A, 0)) == INVALID               # NULL peer pointer
+    assert pcall(dsts=(A, B + 8)) == ALIGN
+    assert pcall(dsts=(A, A)) == OVERLAP               # two peers, one buffer
+    assert pcall(dsts=(A, C + 256)) == OVERLAP         # a destination inside the source
+    assert pcall(Pn=9, H=72, dsts=tuple([A] * 9)) == UNSUPPORTED
+    assert pcall(n=5, srcs=tuple([C] * 5), dsts=tuple([A] * 10)) == UNSUPPORTED
+    assert pcall(dt=4) == UNSUPPORTED
+    assert pcall(n=0) == OK
+    assert pcall(Ls=0, La=0) == OK                     # nothing to move, nothing launched
+
+    bw = lib.ws_kv_slice_broadcast_write
+
+    def bcall(kcs=(A, B), vcs=(C, D), Pn=2, cap=256, Hp=2, d=64, ks=0x50000000, vs=0x60000000, n=8, off=10, dt=0):
+        return bw(arr(*kcs), arr(*vcs), Pn, cap, Hp, d, vp(ks), vp(vs), n, off, dt, None)
+
+    assert bcall(off=250) == RANGE
+    assert bcall(kcs=(A, 0)) == INVALID
+    assert bcall(kcs=(A, A)) == OVERLAP                # two ranks sharing one cache
+    assert bcall(vcs=(C, A)) == OVERLAP
+    assert bcall(ks=A + 1024) == OVERLAP
+    assert bcall(kcs=(A, B + 4)) == ALIGN
+    assert bcall(Pn=9, kcs=tuple([A] * 9), vcs=tuple([C] * 9)) == UNSUPPORTED
+    assert bcall(n=0) == OK
+
+    po = lib.ws_block_causal_attn_push_out
+    Mask = binding._BlockMask
+
+    def ocall(outs=(A, B), Pn=2, rank=1, Ls=30, Lq=64, H=2, d=128, q=C):
+        m = Mask(1, (ctypes.c_int32 * 1)(Lq), (ctypes.c_int32 * 1)(512))
+        return po(arr(*outs), Pn, rank, Ls, None, vp(q), vp(D), vp(0x40000000), 512, 512, None, None, 0, H, d, Lq, ctypes.byref(m), 0.1,
+                  vp(0x70000000), 1 << 30, 0, None)
+
+    assert ocall(rank=2) == INVALID
+    assert ocall(outs=(A, 0)) == INVALID
+    assert ocall(Ls=33) == RANGE                       # P * Ls > Lq
+    assert ocall(outs=(A, A + 64)) == OVERLAP
+    assert ocall(outs=(A, B + 2)) == ALIGN
+    assert ocall(d=96) == UNSUPPORTED
+    assert ocall(Pn=9, outs=tuple([A] * 9), Ls=7) == UNSUPPORTED
+    if not torch.cuda.is_available():
+        assert ocall() == CUDA and pcall() == CUDA and bcall() == CUDA     # valid calls reach CUDA: no CPU fallback
+
+
 def test_unit_forward_host_checks_everything_before_enqueueing(lib):
     """ws_unit_forward_host runs every check of the calls it is made of (cache write, attention) up front, so a call
     that will fail enqueues no copy and forks no helper stream.  On this CPU-only box that is observable: every
