@@ -520,6 +520,85 @@ def fp8_aux(peaks):
     return res
 
 
+def next_rows_aux(peaks):
+    """SURVEY.md 8(f).4 and 8(f).2 on one GPU: config-3 attention on a ring cache whose window has wrapped (against the linear
+    cache), a wrapping ring write, and config 4's Ulysses group with the exchange done as stores into (here: local) peer
+    buffers -- exchange #1 by the pack kernel, exchange #2 by the attention epilogue -- against the plain attention call."""
+    import torch
+    import paper_2607_04443_b200 as ws
+    res = {}
+    g = torch.Generator(device="cuda").manual_seed(9)
+    rnd = lambda std, *s: (torch.randn(*s, generator=g, device="cuda", dtype=torch.float32) * std).to(torch.bfloat16)
+
+    def graph_ms(call, reps=10):
+        for _ in range(2):
+            call()
+        torch.cuda.synchronize()
+        st, cg = torch.cuda.Stream(), torch.cuda.CUDAGraph()
+        with torch.cuda.graph(cg, stream=st):
+            for _ in range(reps):
+                call()
+        cg.replay()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        best = None
+        for _ in range(3):
+            a.record()
+            cg.replay()
+            b.record()
+            torch.cuda.synchronize()
+            t = a.elapsed_time(b) / reps
+            best = t if best is None else min(best, t)
+        return best
+
+    # ---- ring cache: cfg3 shape, the ring exactly as large as the window (16384 rows), 23 units of 970 rows written
+    cfg = wl.CONFIGS["cfg3"]
+    L, H, d, cap = cfg.Lq, cfg.H, cfg.d, cfg.cache_len
+    kc, vc = rnd(1.0, H, cap, d), rnd(1.0, H, cap, d)
+    q, kn, vn = rnd(1.0, L, H, d), rnd(1.0, L, H, d), rnd(1.0, L, H, d)
+    out = torch.empty_like(q)
+    wsp = torch.empty(ws.block_causal_attn_workspace_bytes(L, H, d, cap + L), dtype=torch.uint8, device="cuda")
+    start, clen = ws.ring_state(23 * 970, cap)
+    ms_lin = graph_ms(lambda: ws.block_causal_attn(out, q, kc, vc, cap, kn, vn, [L], [cap + L], cfg.softmax_scale, wsp))
+    ms_ring = graph_ms(lambda: ws.block_causal_attn_ring(out, q, kc, vc, start, clen, kn, vn, [L], [cap + L], cfg.softmax_scale, wsp))
+    res["ring_cfg3"] = {"attention_ms_linear_cache": ms_lin, "attention_ms_ring_cache": ms_ring, "ring_start": start, "cache_len": clen,
+                        "tflops_ring": cfg.attn_flops() / ms_ring / 1e9}
+    ks, vs = rnd(1.0, 970, H, d), rnd(1.0, 970, H, d)
+    ms_w = graph_ms(lambda: ws.kv_cache_write_ring(kc, vc, ks, vs, 0, cap - 400), 50)      # 400 rows at the end, 570 at the start
+    byts = 2 * 2 * 970 * H * d * 2
+    # the same 40 MB every repetition: the payload stays in the 126 MB L2, so this is launch + L2 time, not an HBM figure
+    res["ring_write_970rows_wrapping"] = {"us": ms_w * 1e3, "launches": 2, "gbs_l2_resident": byts / ms_w / 1e6, "bytes": byts}
+    del kc, vc, q, kn, vn, out, wsp, ks, vs
+
+    # ---- Ulysses group, cfg4 geometry: P = 4 ranks, 4 x 920 video tokens + 50 audio tokens, 40 heads (10 per rank)
+    P, Ls, La, Ht, Hp, Tc = 4, 920, 50, 40, 10, 16384
+    Lq = P * Ls + La
+    xs = [rnd(1.0, Ls + La, Ht, d) for _ in range(3)]                                         # one rank's Q, K_new, V_new shard
+    ys = [[torch.empty((Lq, Hp, d), dtype=torch.bfloat16, device="cuda") for _ in range(P)] for _ in range(3)]
+    ms_push = graph_ms(lambda: ws.ulysses_push_seq_to_head(ys, xs, Ls, 1), 50)
+    byts = 2 * 3 * (Ls + La // P) * Ht * d * 2
+    res["ulysses_push_seq_to_head_rank"] = {"us": ms_push * 1e3, "bytes": byts, "gbs_l2_resident": byts / ms_push / 1e6, "launches": 2,
+                                            "what": "one rank's Q, K_new, V_new shards (920 + 50 tokens x 40 heads) packed into 4 peers' buffers (local stand-ins)"}
+    kc, vc = rnd(1.0, Hp, Tc, d), rnd(1.0, Hp, Tc, d)
+    for t in ys[0] + ys[1] + ys[2]:
+        t.copy_(rnd(1.0, Lq, Hp, d))
+    zs = [torch.empty((Ls + La, Ht, d), dtype=torch.bfloat16, device="cuda") for _ in range(P)]
+    o = torch.empty((Lq, Hp, d), dtype=torch.bfloat16, device="cuda")
+    wsp = torch.empty(ws.block_causal_attn_workspace_bytes(Lq, Hp, d, Tc + Lq), dtype=torch.uint8, device="cuda")
+    qe = [Ls, 2 * Ls, 3 * Ls, Lq]
+    kv = [Tc + e for e in qe]
+    ms_plain = graph_ms(lambda: ws.block_causal_attn(o, ys[0][1], kc, vc, Tc, ys[1][1], ys[2][1], qe, kv, cfg.softmax_scale, wsp))
+    ms_po = graph_ms(lambda: ws.block_causal_attn_push_out(zs, 1, Ls, ys[0][1], kc, vc, Tc, ys[1][1], ys[2][1], qe, kv, cfg.softmax_scale, wsp))
+    res["ulysses_attention_rank"] = {"ms_plain_attention": ms_plain, "ms_attention_with_exchange2_in_epilogue": ms_po,
+                                     "what": "rank 1 of 4: 3730 queries x 10 heads, 16384 cached rows; O rows stored to 4 peers' token-major outputs"}
+    kcs, vcs = [rnd(1.0, Hp, Tc, d) for _ in range(P)], [rnd(1.0, Hp, Tc, d) for _ in range(P)]
+    ks, vs = rnd(1.0, 1024, Ht, d), rnd(1.0, 1024, Ht, d)
+    ms_b = graph_ms(lambda: ws.kv_slice_broadcast_write(kcs, vcs, ks, vs, 15360), 50)
+    byts = 2 * 2 * 1024 * Ht * d * 2
+    res["kv_slice_broadcast_write_4ranks"] = {"us": ms_b * 1e3, "bytes": byts, "gbs_l2_resident": byts / ms_b / 1e6, "launches": 1}
+    return res
+
+
 def run_fp8_kernels_only(args):
     """cfg3 through the FP8-cache calls, for ncu: slice write + attention, args.warmup + args.steps times."""
     import torch
@@ -658,7 +737,8 @@ def run_ours(args):
             del unit
             torch.cuda.empty_cache()
             aux = {"hbm_peak_gbs": peaks["hbm_gbs"], "peak_source": peaks["_source"]}
-            for key, fn in (("attention", attention_aux), ("fp8_kv_cache", fp8_aux), ("bandwidth", bandwidth_aux)):
+            for key, fn in (("attention", attention_aux), ("fp8_kv_cache", fp8_aux), ("ring_and_ulysses", next_rows_aux),
+                            ("bandwidth", bandwidth_aux)):
                 aux[key] = fn(peaks)
                 torch.cuda.synchronize()
                 torch.cuda.empty_cache()
