@@ -42,6 +42,7 @@ def build_lib(force: bool = False, verbose: bool = False) -> str:
         return LIB
     tmp = LIB + f".tmp{os.getpid()}"
     cmd = [_nvcc()] + NVCC_FLAGS + ["-I", os.path.join(ROOT, "include"), "-I", CSRC]
+    cmd += os.environ.get("WS_NVCC_EXTRA", "").split()  # e.g. -DWS_CHUNK_ENDS=2468 for a tuning build
     if verbose:
         cmd += ["-Xptxas", "-v"]
     cmd += ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]

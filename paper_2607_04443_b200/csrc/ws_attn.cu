@@ -72,14 +72,17 @@ constexpr int kTmemCols = 512;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kRescaleThreshold = 8.0f;  // log2 units: P stays below 2^8
-#ifndef WS_POLY_OF4
-#define WS_POLY_OF4 1
+// Which exponentials run on the FMA pipe (degree-3 polynomial) instead of MUFU: bit (u & 1) * 8 + i of the mask selects pair i
+// (2 keys) of the 16-key unit u.  0x1111 = pairs 0 and 4 of every unit = 1 exponential in 4.  The optimum is flat on B200:
+// 1/8 .. 3/8 are within 1 % of each other (profiles/r02b_attn_variants.md); all-MUFU and 1/2 are 2-3 % slower.
+#ifndef WS_POLY_MASK
+#define WS_POLY_MASK 0x1111
 #endif
-constexpr int kPolyOf4 = WS_POLY_OF4;
+constexpr unsigned kPolyMask = WS_POLY_MASK;
 #ifndef WS_WARP_ARRIVE
 #define WS_WARP_ARRIVE 0
 #endif
-constexpr int kPReadyArrivals = WS_WARP_ARRIVE ? 4 : 128;  // arrivals per P-chunk barrier: one per softmax warp, or one per thread  // of every 4 pairs of exponentials, this many run on the FMA pipe instead of MUFU
+constexpr int kPReadyArrivals = WS_WARP_ARRIVE ? 4 : 128;  // arrivals per P-chunk barrier: one per softmax warp, or one per thread
 
 struct alignas(64) Params {
   CUtensorMap map_q, map_kn, map_vn, map_kc, map_vc;
@@ -118,6 +121,7 @@ struct alignas(64) Params {
   // remaining items [n_waves * grid, H * n_units) are split stream-K style, CTA c taking the flattened
   // iterations [pool_begin[c], pool_begin[c + 1]) (global coordinates head * Tp + unit_prefix).
   int32_t n_waves, grid;
+  int32_t combine_items;  // pool items the combine kernel has work for: split over several CTAs, or without any visible key (0: not launched)
   int64_t pool_begin[kMaxCtas + 1];
 };
 
@@ -177,6 +181,10 @@ __device__ __forceinline__ int cta_of_iter(const Params& p, int64_t t) {
   }
   return lo;
 }
+
+// CTA c takes no pool iteration: the cost-aware partition leaves a CTA empty when its phase-1 items were the expensive
+// ones.  Such a CTA may sit INSIDE the CTA span of a split item; it writes no partial record.
+__device__ __forceinline__ bool pool_empty(const Params& p, int c) { return p.pool_begin[c] == p.pool_begin[c + 1]; }
 
 struct Segment {
   int head, unit, i0, i1, n_iters;  // iterations [i0, i1) of the unit's n_iters
@@ -760,7 +768,7 @@ __global__ void __launch_bounds__(KV8 ? kThreads8 : kThreads, 1) attn_fwd_kernel
         const float2 sc2 = make_float2(p.scale_log2, p.scale_log2), nm2 = make_float2(neg_ms, neg_ms);
         float2 sumA = make_float2(0.f, 0.f), sumB = make_float2(0.f, 0.f);
         auto exp_halves = [&](auto poly_tag) {
-          constexpr int kPoly = decltype(poly_tag)::value;
+          constexpr unsigned kPoly = decltype(poly_tag)::value;
 #pragma unroll
           for (int u = 0; u < kBlockN / 16; ++u) {  // 16 keys -> 8 packed BF16 pairs -> 8 TMEM columns
             uint32_t pk[8];
@@ -769,7 +777,7 @@ __global__ void __launch_bounds__(KV8 ? kThreads8 : kThreads, 1) attn_fwd_kernel
               const int key = u * 16 + 2 * i;
               const float2 x = ptx::fma2(make_float2(__uint_as_float(s[key >> 5][key & 31]), __uint_as_float(s[key >> 5][(key & 31) + 1])), sc2, nm2);
               float2 e;
-              if ((i & 3) < kPoly) e = ptx::ex2_poly2(x);
+              if ((kPoly >> ((u & 1) * 8 + i)) & 1u) e = ptx::ex2_poly2(x);
               else e = make_float2(ptx::ex2(x.x), ptx::ex2(x.y));
               if (i & 1) sumB = ptx::add2(sumB, e); else sumA = ptx::add2(sumA, e);
               pk[i] = ptx::pack_bf16(e.x, e.y);
@@ -782,8 +790,8 @@ __global__ void __launch_bounds__(KV8 ? kThreads8 : kThreads, 1) attn_fwd_kernel
             }
           }
         };
-        if (__any_sync(0xffffffffu, lim < kBlockN)) exp_halves(std::integral_constant<int, 0>{});
-        else exp_halves(std::integral_constant<int, kPolyOf4>{});
+        if (__any_sync(0xffffffffu, lim < kBlockN)) exp_halves(std::integral_constant<unsigned, 0u>{});
+        else exp_halves(std::integral_constant<unsigned, kPolyMask>{});
         const float2 sum2 = ptx::add2(sumA, sumB);
         l += sum2.x + sum2.y;
       }
@@ -894,7 +902,7 @@ __global__ void __launch_bounds__(kPairM) attn_combine_kernel(const __grid_const
       for (int u = 0; u < kBatch; ++u) {
         ml[u] = make_float2(-INFINITY, 0.f);
         o[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (k + u < n_rec) {
+        if (k + u < n_rec && !pool_empty(p, c_lo + (single ? (k + u) >> 1 : k + u))) {  // an empty CTA inside the span wrote no record
           const int64_t rec = rec0 + (int64_t)(k + u) * stride;
           ml[u] = p.part_ml[rec * kBlockM + r];
           o[u] = reinterpret_cast<const float4*>(p.part_o)[(rec * (D / 4) + q4) * kBlockM + r];
@@ -1077,7 +1085,7 @@ int launch_attention(const Params& prm, DeviceState* st, cudaStream_t stream) {
     ++launches;
   }
   const int n_pool_items = prm.H * prm.n_units - prm.n_waves * prm.grid;
-  if (n_pool_items > 0) {
+  if (n_pool_items > 0 && prm.combine_items > 0) {
     dim3 cgrid((unsigned)n_pool_items, D / 4);  // items on x: H * n_units may exceed the 65535 limit of y
     const cudaError_t e = wsi::launch_pdl(attn_combine_kernel<D, OUT_F32>, cgrid, dim3(kPairM), 0, stream, prm);
     if (e != cudaSuccess) return wsi::cuda_fail(e);
@@ -1183,7 +1191,32 @@ bool partition_pool(const Params& prm, int64_t Tp, int64_t t_begin, int64_t T, i
   return t == T;
 }
 
-// The two-phase schedule (see Params) for a device with `sms` SMs: fills prm.grid, n_waves, pool_begin.
+// Pool items the combine kernel has work for: those that see no key (zero fill) and those split over several CTAs.
+// Fills prm.combine_items (0: the combine kernel is not launched).
+void count_combine_items(Params& prm) {
+  const int n_units = prm.n_units;
+  const int64_t n_items = (int64_t)prm.H * n_units, Tp = prm.unit_prefix[n_units];
+  const int G = prm.grid;
+  auto cta_of = [&](int64_t t) {
+    int lo = 0, hi = G - 1;
+    while (lo < hi) {
+      const int mid = (lo + hi + 1) >> 1;
+      if (prm.pool_begin[mid] <= t) lo = mid; else hi = mid - 1;
+    }
+    return lo;
+  };
+  int32_t n = 0;
+  for (int64_t w = (int64_t)prm.n_waves * G; w < n_items; ++w) {
+    const int u = (int)(w % n_units);
+    const int64_t iters = prm.unit_prefix[u + 1] - prm.unit_prefix[u];
+    if (iters == 0) { ++n; continue; }
+    const int64_t a = (w / n_units) * Tp + prm.unit_prefix[u];
+    if (cta_of(a + iters - 1) != cta_of(a)) ++n;
+  }
+  prm.combine_items = n;
+}
+
+// The two-phase schedule (see Params) for a device with `sms` SMs: fills prm.grid, n_waves, pool_begin, combine_items.
 void build_schedule(Params& prm, int64_t Tp, int sms) {
   const int n_units = prm.n_units, H = prm.H;
   const int64_t T = Tp * H, n_items = (int64_t)H * n_units;
@@ -1194,6 +1227,7 @@ void build_schedule(Params& prm, int64_t Tp, int sms) {
   if (T == 0) {  // nothing visible anywhere: every item is a (zero-filling) phase-1 item
     prm.n_waves = (int32_t)((n_items + G - 1) / G);
     for (int64_t c = 0; c <= G; ++c) prm.pool_begin[c] = 0;
+    prm.combine_items = 0;
     return;
   }
   auto item_cost = [&](int64_t i) {
@@ -1252,6 +1286,7 @@ void build_schedule(Params& prm, int64_t Tp, int sms) {
   }
   prm.n_waves = use_b ? (int32_t)W : 0;
   for (int64_t c = 0; c <= G; ++c) prm.pool_begin[c] = use_b ? begin_b[c] : begin_a[c];
+  count_combine_items(prm);
 }
 
 // The schedule depends on the problem shape only (Lq, H, cache_len, Ln, mask, SM count): a streaming session repeats
@@ -1265,7 +1300,7 @@ struct ScheduleEntry {
   bool valid = false;
   uint64_t stamp = 0;
   ScheduleKey key;
-  int32_t n_cache_tiles, n_tiles_a, last_single, last_kv_tiles, n_waves, grid;
+  int32_t n_cache_tiles, n_tiles_a, last_single, last_kv_tiles, n_waves, grid, combine_items;
   int64_t len_a;
   int32_t unit_prefix[kMaxUnits + 1];
   int64_t pool_begin[kMaxCtas + 1];
@@ -1286,7 +1321,7 @@ int64_t schedule_for(Params& prm, const ws_block_mask* mask, int sms) {
       e.stamp = ++clock;
       prm.n_cache_tiles = e.n_cache_tiles; prm.n_tiles_a = e.n_tiles_a; prm.len_a = e.len_a;
       prm.last_single = e.last_single; prm.last_kv_tiles = e.last_kv_tiles;
-      prm.n_waves = e.n_waves; prm.grid = e.grid;
+      prm.n_waves = e.n_waves; prm.grid = e.grid; prm.combine_items = e.combine_items;
       memcpy(prm.unit_prefix, e.unit_prefix, sizeof(int32_t) * (prm.n_units + 1));
       memcpy(prm.pool_begin, e.pool_begin, sizeof(int64_t) * (e.grid + 1));
       return prm.unit_prefix[prm.n_units];
@@ -1298,7 +1333,7 @@ int64_t schedule_for(Params& prm, const ws_block_mask* mask, int sms) {
   victim->valid = true; victim->stamp = ++clock; victim->key = key;
   victim->n_cache_tiles = prm.n_cache_tiles; victim->n_tiles_a = prm.n_tiles_a; victim->len_a = prm.len_a;
   victim->last_single = prm.last_single; victim->last_kv_tiles = prm.last_kv_tiles;
-  victim->n_waves = prm.n_waves; victim->grid = prm.grid;
+  victim->n_waves = prm.n_waves; victim->grid = prm.grid; victim->combine_items = prm.combine_items;
   memcpy(victim->unit_prefix, prm.unit_prefix, sizeof(int32_t) * (prm.n_units + 1));
   memcpy(victim->pool_begin, prm.pool_begin, sizeof(int64_t) * (prm.grid + 1));
   return Tp;

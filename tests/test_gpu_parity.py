@@ -641,3 +641,71 @@ def test_unit_forward_host_degenerate_key_sources(Tc0, n_w, Ln):
     check_attn(got, ref, what=f"host entry Tc0={Tc0} n_w={n_w} Ln={Ln}")
     if Tc + Ln == 0:
         assert np.all(got == 0.0)
+
+
+# ================================================================================================
+# split work items: partial records, combine kernel, scratch workspace
+# ================================================================================================
+def attention_with_workspace_fill(c, fill):
+    """The plain call, with the workspace pre-filled by `fill(workspace)` (its contents are scratch by contract)."""
+    tq, tkc, tvc = to_dev(c["q"], "bf16"), to_dev(c["k_cache"], "bf16"), to_dev(c["v_cache"], "bf16")
+    tkn = to_dev(c["k_new"], "bf16") if c["k_new"] is not None else None
+    tvn = to_dev(c["v_new"], "bf16") if c["v_new"] is not None else None
+    Lq, H, d = c["q"].shape
+    Ln = 0 if tkn is None else tkn.shape[0]
+    out = torch.full_like(tq, float("nan"))
+    lse = torch.full((H, Lq), float("nan"), dtype=torch.float32, device="cuda")
+    wsp = workspace_for(Lq, H, d, c["cache_len"] + Ln)
+    fill(wsp)
+    ws.block_causal_attn(out, tq, tkc, tvc, c["cache_len"], tkn, tvn, list(c["q_block_end"]), list(c["kv_visible"]), c["scale"], wsp, lse=lse)
+    torch.cuda.synchronize()
+    return to_host(out), lse.cpu().numpy()
+
+
+@pytest.mark.parametrize("Lq,H,Tc", [(268, 79, 300), (893, 40, 300), (369, 79, 1000)])
+def test_split_item_whose_cta_span_contains_an_empty_cta(Lq, H, Tc):
+    """Shapes for which (on 148 SMs) the cost-aware partition leaves a CTA without pool work INSIDE the CTA span of a split
+    item: that CTA writes no partial record, and the merge must not read one.  The workspace is filled with NaN bytes so a
+    stale read cannot pass by luck."""
+    c = rand_case(Lq + H, H, 128, [Lq], [Tc], Tc, 0)
+    got, got_lse = attention_with_workspace_fill(c, lambda w: w.fill_(0xFF))
+    ref, ref_lse = wsref.block_causal_attn(c["q"], c["k_cache"], c["v_cache"], Tc, None, None, c["q_block_end"], c["kv_visible"], c["scale"])
+    check_attn(got, ref, got_lse, ref_lse, what=f"Lq={Lq} H={H} Tc={Tc}")
+
+
+@pytest.mark.parametrize("fill", ["zeros", "ones", "random"])
+def test_workspace_contents_are_scratch(fill):
+    """The split-KV partial records live in the caller's workspace, whose contents are scratch: it may hold anything."""
+    c = rand_case(77, 24, 128, [292], [2048 + 292], 2048, 292)          # config-2-like: every item is split over several CTAs
+    fills = {"zeros": lambda w: w.zero_(), "ones": lambda w: w.fill_(0xFF),
+             "random": lambda w: w.copy_(torch.randint(0, 256, w.shape, dtype=torch.uint8, device="cuda"))}
+    got, got_lse = attention_with_workspace_fill(c, fills[fill])
+    ref, ref_lse = wsref.block_causal_attn(c["q"], c["k_cache"], c["v_cache"], 2048, c["k_new"], c["v_new"], c["q_block_end"],
+                                           c["kv_visible"], c["scale"])
+    check_attn(got, ref, got_lse, ref_lse, what=fill)
+
+
+def test_graph_replays_of_a_split_item_shape():
+    """Two calls that share one workspace inside one CUDA graph, replayed with fresh queries: every replay must stand on its
+    own (no state survives in the workspace from one call or replay to the next)."""
+    c = rand_case(78, 10, 128, [700], [1500 + 700], 1500, 700)
+    tq, tkc, tvc = to_dev(c["q"], "bf16"), to_dev(c["k_cache"], "bf16"), to_dev(c["v_cache"], "bf16")
+    tkn, tvn = to_dev(c["k_new"], "bf16"), to_dev(c["v_new"], "bf16")
+    out = torch.empty_like(tq)
+    wsp = workspace_for(700, 10, 128, 2200)
+    args = (tkc, tvc, 1500, tkn, tvn, [700], [2200], c["scale"], wsp)
+    ws.block_causal_attn(out, tq, *args)
+    torch.cuda.synchronize()
+    st, cg = torch.cuda.Stream(), torch.cuda.CUDAGraph()
+    with torch.cuda.graph(cg, stream=st):
+        ws.block_causal_attn(out, tq, *args)
+        ws.block_causal_attn(out, tq, *args)      # two calls in one graph share the workspace
+    rng = np.random.default_rng(5)
+    for rep in range(4):
+        q = wl.bf16_round(rng.standard_normal(c["q"].shape, dtype=np.float32))
+        tq.copy_(to_dev(q, "bf16"))
+        out.fill_(float("nan"))
+        cg.replay()
+        torch.cuda.synchronize()
+        ref, _ = wsref.block_causal_attn(q, c["k_cache"], c["v_cache"], 1500, c["k_new"], c["v_new"], [700], [2200], c["scale"])
+        check_attn(to_host(out), ref, what=f"replay {rep}")

@@ -137,3 +137,28 @@ def test_schedule_rejects_bad_masks():
     with pytest.raises(ws.WsError) as e:
         ws.attn_schedule(100, 2, 50, 0, [60, 100], [40, 30], 148)  # kv_visible must not decrease
     assert e.value.status == -1
+
+
+@pytest.mark.parametrize("Lq,H,Tc", [(268, 79, 300), (893, 40, 300), (369, 79, 1000)])
+def test_schedules_with_an_empty_cta_inside_a_split_items_span_exist(Lq, H, Tc):
+    """The cost-aware partition may leave a CTA without pool iterations while its neighbours on both sides hold pieces of
+    the same split item (its whole-item wave was the expensive one).  The attention kernel writes one partial record per
+    CTA that holds a piece, so the merge must skip such a CTA (tests/test_gpu_parity.py has the GPU side of these shapes,
+    which produced wrong rows before the merge learnt to).  This pins the premise on the host."""
+    import bisect
+    plan = ws.attn_schedule(Lq, H, Tc, 0, [Lq], [Tc], 148)
+    pool, grid, iters = plan["pool_begin"], plan["grid"], plan["unit_iters"]
+    n_units, Tp = len(iters), sum(iters)
+    prefix = [0]
+    for t in iters:
+        prefix.append(prefix[-1] + t)
+    cta_of = lambda t: bisect.bisect_right(pool, t, 0, grid) - 1
+    hit = False
+    for w in range(plan["n_waves"] * grid, H * n_units):
+        u = w % n_units
+        if iters[u] == 0:
+            continue
+        a = (w // n_units) * Tp + prefix[u]
+        lo, hi = cta_of(a), cta_of(a + iters[u] - 1)
+        hit |= any(pool[c] == pool[c + 1] for c in range(lo, hi + 1))
+    assert hit
