@@ -73,10 +73,12 @@ constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kRescaleThreshold = 8.0f;  // log2 units: P stays below 2^8
 // Which exponentials run on the FMA pipe (degree-3 polynomial) instead of MUFU: bit (u & 1) * 8 + i of the mask selects pair i
-// (2 keys) of the 16-key unit u.  0x1111 = pairs 0 and 4 of every unit = 1 exponential in 4.  The optimum is flat on B200:
-// 1/8 .. 3/8 are within 1 % of each other (profiles/r02b_attn_variants.md); all-MUFU and 1/2 are 2-3 % slower.
+// (2 keys) of the 16-key unit u.  0x4949 = pairs 0, 3 and 6 of every unit = 3 exponentials in 8.  Measured on B200 (cfg3,
+// profiles/r02b_attn_variants.md): the share has a flat optimum between 1/8 and 3/8, but the POSITIONS matter as much as the
+// share (they decide how ptxas interleaves the MUFU and FMA chains): 0x4949 is 1.5 % faster than 0x1111 (1 in 4), another
+// 3-in-8 pattern (0x2592) is no better than 0x1111, 1 in 2 (0x5555) is 4 % slower.
 #ifndef WS_POLY_MASK
-#define WS_POLY_MASK 0x1111
+#define WS_POLY_MASK 0x4949
 #endif
 constexpr unsigned kPolyMask = WS_POLY_MASK;
 #ifndef WS_WARP_ARRIVE
