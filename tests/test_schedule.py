@@ -109,11 +109,13 @@ def test_every_step_is_assigned_exactly_once_and_loads_are_balanced(case):
     assert all(qt % 2 == 0 and qt + 1 < n_q_tiles for _, qt, _ in extra), "only a pair's earlier tile may run invisible tiles"
     assert sum(load) == T
     # balance, in the schedule's cost model: no CTA exceeds the even share of the unavoidable cost (every iteration, one
-    # segment per non-empty item) by more than 3 % plus what contiguity can strand (two segments and an iteration)
+    # segment per non-empty item) by more than 6 % plus what contiguity can strand (two segments and an iteration).  6 % is the
+    # slack the scheduler grants whole-item waves over pure stream-K: they write far fewer partials, which the model does not
+    # price (measured on B200, config 4: modelled 4-5 % longer, 3.5 % faster)
     if T:
         single_last = n_q_tiles % 2 == 1
         unavoidable = H * sum((200 + n * 100) for u, n in enumerate(want_iters) if n)
-        assert max(cost) <= math.ceil(unavoidable / plan["grid"]) * 1.03 + 2 * 200 + 100
+        assert max(cost) <= math.ceil(unavoidable / plan["grid"]) * 1.06 + 2 * 200 + 100
 
 
 def test_baseline_configs_take_the_documented_schedules():
@@ -124,7 +126,8 @@ def test_baseline_configs_take_the_documented_schedules():
     assert (p3["grid"], p3["n_waves"], p3["unit_iters"]) == (148, 1, [136] * 4)       # 148 whole items + 12 split ones
     assert p3["pool_begin"][0] == 37 * 4 * 136 and p3["pool_begin"][-1] == 160 * 136
     assert (p5["grid"], p5["n_waves"]) == (148, 1)
-    assert p4["n_waves"] == 0 and p4["pool_begin"][-1] == 10 * sum(p4["unit_iters"])   # unequal items: pure stream-K
+    # cfg4: unequal items (143 .. 157 iterations, the single 79): one wave of whole items, the last 2 of the 150 items pooled
+    assert (p4["grid"], p4["n_waves"]) == (148, 1) and p4["pool_begin"][-1] == 10 * sum(p4["unit_iters"])
     assert len(p4["unit_iters"]) == 15 and p4["unit_iters"][-1] == (p4["unit_kv_tiles"][-1] + 1) // 2  # 29 Q tiles: 14 pairs + a single
     # cfg2: 292 rows = a pair (67 KV tiles) and a single tile that walks its 67 KV tiles two per iteration
     assert p2["n_waves"] == 0 and p2["unit_iters"] == [67, 34] and p2["unit_kv_tiles"] == [67, 67]
