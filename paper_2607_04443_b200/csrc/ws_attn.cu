@@ -124,6 +124,7 @@ struct alignas(64) Params {
   // iterations [pool_begin[c], pool_begin[c + 1]) (global coordinates head * Tp + unit_prefix).
   int32_t n_waves, grid;
   int32_t combine_items;  // pool items the combine kernel has work for: split over several CTAs, or without any visible key (0: not launched)
+  int32_t combine_max_rec;  // most partial records any of them has per output row
   int64_t pool_begin[kMaxCtas + 1];
 };
 
@@ -871,7 +872,7 @@ __global__ void __launch_bounds__(KV8 ? kThreads8 : kThreads, 1) attn_fwd_kernel
 // that see no key at all.  grid = (number of phase-2 units, d/4), block = 256 threads: thread r handles
 // row r % 128 of tile slot r / 128 (a single unit has one Q tile: its slot-1 threads have nothing to do).
 // ---------------------------------------------------------------------------------------------
-template <int D, bool OUT_F32>
+template <int D, bool OUT_F32, int kBatch>
 __global__ void __launch_bounds__(kPairM) attn_combine_kernel(const __grid_constant__ Params p) {
   wsi::pdl_trigger();
   wsi::pdl_wait();  // the partials are the attention kernel's
@@ -893,9 +894,9 @@ __global__ void __launch_bounds__(kPairM) attn_combine_kernel(const __grid_const
     // slots' records of every CTA (stride 1)
     const int64_t rec0 = ((int64_t)w + c_lo) * 2 + (single ? 0 : slot);
     const int n_rec = (c_hi - c_lo + 1) * (single ? 2 : 1), stride = single ? 1 : 2;
-    // online LSE-weighted merge, four partials per step with all eight loads of a step in flight at once (the kernel
-    // is a chain of dependent L2 round trips otherwise; eight partials per step cost occupancy and measured slower)
-    constexpr int kBatch = 4;
+    // online LSE-weighted merge, kBatch partials per step with all 2 kBatch loads of a step in flight at once (the kernel is a
+    // chain of dependent L2 round trips otherwise).  Four per step when every item has few partials (cfg2, cfg4: eight cost
+    // occupancy and measured slower there), eight when some item has more than eight (cfg3, cfg5: 12-13 partials per item).
     float M = -INFINITY, L = 0.f;
     for (int k = 0; k < n_rec; k += kBatch) {
       float2 ml[kBatch];
@@ -1075,6 +1076,9 @@ WsLayout ws_layout(int32_t Lq, int32_t H, int32_t d, int64_t kv_total, int64_t c
   return L;
 }
 
+#ifndef WS_COMBINE_BATCH8_FROM
+#define WS_COMBINE_BATCH8_FROM 9
+#endif
 template <int D, bool OUT_F32, bool KV8>
 int launch_attention(const Params& prm, DeviceState* st, cudaStream_t stream) {
   using C = Cfg<D, KV8>;
@@ -1089,7 +1093,8 @@ int launch_attention(const Params& prm, DeviceState* st, cudaStream_t stream) {
   const int n_pool_items = prm.H * prm.n_units - prm.n_waves * prm.grid;
   if (n_pool_items > 0 && prm.combine_items > 0) {
     dim3 cgrid((unsigned)n_pool_items, D / 4);  // items on x: H * n_units may exceed the 65535 limit of y
-    const cudaError_t e = wsi::launch_pdl(attn_combine_kernel<D, OUT_F32>, cgrid, dim3(kPairM), 0, stream, prm);
+    const cudaError_t e = prm.combine_max_rec >= WS_COMBINE_BATCH8_FROM ? wsi::launch_pdl(attn_combine_kernel<D, OUT_F32, 8>, cgrid, dim3(kPairM), 0, stream, prm)
+                                                  : wsi::launch_pdl(attn_combine_kernel<D, OUT_F32, 4>, cgrid, dim3(kPairM), 0, stream, prm);
     if (e != cudaSuccess) return wsi::cuda_fail(e);
     ++launches;
   }
@@ -1207,15 +1212,21 @@ void count_combine_items(Params& prm) {
     }
     return lo;
   };
-  int32_t n = 0;
+  int32_t n = 0, max_rec = 0;
   for (int64_t w = (int64_t)prm.n_waves * G; w < n_items; ++w) {
     const int u = (int)(w % n_units);
     const int64_t iters = prm.unit_prefix[u + 1] - prm.unit_prefix[u];
     if (iters == 0) { ++n; continue; }
     const int64_t a = (w / n_units) * Tp + prm.unit_prefix[u];
-    if (cta_of(a + iters - 1) != cta_of(a)) ++n;
+    const int span = cta_of(a + iters - 1) - cta_of(a) + 1;
+    if (span > 1) {
+      ++n;
+      const int rec = span * ((prm.last_single && u == n_units - 1) ? 2 : 1);
+      max_rec = rec > max_rec ? rec : max_rec;
+    }
   }
   prm.combine_items = n;
+  prm.combine_max_rec = max_rec;
 }
 
 // The two-phase schedule (see Params) for a device with `sms` SMs: fills prm.grid, n_waves, pool_begin, combine_items.
@@ -1230,6 +1241,7 @@ void build_schedule(Params& prm, int64_t Tp, int sms) {
     prm.n_waves = (int32_t)((n_items + G - 1) / G);
     for (int64_t c = 0; c <= G; ++c) prm.pool_begin[c] = 0;
     prm.combine_items = 0;
+    prm.combine_max_rec = 0;
     return;
   }
   auto item_cost = [&](int64_t i) {
@@ -1304,7 +1316,7 @@ struct ScheduleEntry {
   bool valid = false;
   uint64_t stamp = 0;
   ScheduleKey key;
-  int32_t n_cache_tiles, n_tiles_a, last_single, last_kv_tiles, n_waves, grid, combine_items;
+  int32_t n_cache_tiles, n_tiles_a, last_single, last_kv_tiles, n_waves, grid, combine_items, combine_max_rec;
   int64_t len_a;
   int32_t unit_prefix[kMaxUnits + 1];
   int64_t pool_begin[kMaxCtas + 1];
@@ -1325,7 +1337,7 @@ int64_t schedule_for(Params& prm, const ws_block_mask* mask, int sms) {
       e.stamp = ++clock;
       prm.n_cache_tiles = e.n_cache_tiles; prm.n_tiles_a = e.n_tiles_a; prm.len_a = e.len_a;
       prm.last_single = e.last_single; prm.last_kv_tiles = e.last_kv_tiles;
-      prm.n_waves = e.n_waves; prm.grid = e.grid; prm.combine_items = e.combine_items;
+      prm.n_waves = e.n_waves; prm.grid = e.grid; prm.combine_items = e.combine_items; prm.combine_max_rec = e.combine_max_rec;
       memcpy(prm.unit_prefix, e.unit_prefix, sizeof(int32_t) * (prm.n_units + 1));
       memcpy(prm.pool_begin, e.pool_begin, sizeof(int64_t) * (e.grid + 1));
       return prm.unit_prefix[prm.n_units];
@@ -1337,7 +1349,7 @@ int64_t schedule_for(Params& prm, const ws_block_mask* mask, int sms) {
   victim->valid = true; victim->stamp = ++clock; victim->key = key;
   victim->n_cache_tiles = prm.n_cache_tiles; victim->n_tiles_a = prm.n_tiles_a; victim->len_a = prm.len_a;
   victim->last_single = prm.last_single; victim->last_kv_tiles = prm.last_kv_tiles;
-  victim->n_waves = prm.n_waves; victim->grid = prm.grid; victim->combine_items = prm.combine_items;
+  victim->n_waves = prm.n_waves; victim->grid = prm.grid; victim->combine_items = prm.combine_items; victim->combine_max_rec = prm.combine_max_rec;
   memcpy(victim->unit_prefix, prm.unit_prefix, sizeof(int32_t) * (prm.n_units + 1));
   memcpy(victim->pool_begin, prm.pool_begin, sizeof(int64_t) * (prm.grid + 1));
   return Tp;
