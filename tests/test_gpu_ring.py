@@ -208,6 +208,27 @@ def test_streaming_session_config3_sized_window_that_has_wrapped():
     check(to_host(out), lse.cpu().numpy(), ref, ref_lse, "session")
 
 
+def test_config3_full_size_on_a_wrapped_ring_whole_tensor():
+    """BASELINE.json config 3 at full size (970 queries x 40 heads, 16384 cached rows + the unit's own 970), the cache held as a
+    16384-row ring whose window starts at an unaligned row: whole [Lq, H, d] tensor and LSE against the FP64 oracle on the
+    linearised window -- the launch configuration bench.py times in aux.ring_and_ulysses.ring_cfg3."""
+    cfg = wl.CONFIGS["cfg3"]
+    x = wl.generate(cfg)
+    kc, vc = x["k_cache"].copy(), x["v_cache"].copy()
+    wsref.kv_cache_write(kc, vc, x["k_slice"], x["v_slice"], 0, cfg.write_offset)          # the linear timeline: 16384 valid rows
+    cap = cfg.cache_len
+    start = ws.ring_state(23 * 970, cap)[0]
+    assert start % 128 != 0
+    ring_k = np.ascontiguousarray(np.roll(kc[:, :cap], start, axis=1))                      # timeline row j sits at (start + j) % cap
+    ring_v = np.ascontiguousarray(np.roll(vc[:, :cap], start, axis=1))
+    q, kn, vn = x["q"][0], x["k_new"][0], x["v_new"][0]
+    got, got_lse = gpu_ring_attention(q, ring_k, ring_v, start, cap, kn, vn, cfg.q_block_end, cfg.kv_visible, cfg.softmax_scale)
+    ref, ref_lse = wsref.block_causal_attn(q, kc, vc, cap, kn, vn, cfg.q_block_end, cfg.kv_visible, cfg.softmax_scale)
+    check(got, got_lse, ref, ref_lse, "cfg3 on a ring")
+    # and the ring oracle agrees with the linear one on this window (the roll above is the inverse of its linearisation)
+    assert np.array_equal(wsref_ring.linearise(ring_k, start, cap), kc[:, :cap])
+
+
 def test_ring_attention_errors_launch_nothing():
     H, d, cap = 2, 128, 256
     q = torch.zeros((16, H, d), dtype=torch.bfloat16, device="cuda")

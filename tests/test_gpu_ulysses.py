@@ -194,6 +194,36 @@ def test_config4_sized_group_whole_pipeline():
         assert ma <= MAX_ABS and rf <= REL_FRO, f"rank {r}: max_abs={ma:.3e} rel_fro={rf:.3e}"
 
 
+def test_config4_full_width_rank_against_the_oracle():
+    """One rank of config 4's group at FULL width -- 10 heads, 4 x 920 + 50 queries, 16384 cached rows, four causal blocks --
+    through exchange #1, attention with exchange #2 in its epilogue, against the FP64 oracle on that rank's heads: the launch
+    configuration bench.py times in aux.ring_and_ulysses.ulysses_attention_rank."""
+    rng = np.random.default_rng(21)
+    P, Ls, La, Hp, d, Tc, g = 4, 920, 50, 10, 128, 16384, 1
+    H, L = P * Hp, P * Ls + La
+    q_r, k_r, v_r = (make_rank_inputs(rng, P, Ls, La, H, d, "bf16") for _ in range(3))
+    kc, vc = gen(rng, "bf16", Hp, Tc, d), gen(rng, "bf16", Hp, Tc, d)
+    qe = [Ls, 2 * Ls, 3 * Ls, L]
+    kv = [Tc + e for e in qe]
+    scale = 1.0 / math.sqrt(d)
+    ys = [[torch.empty((L, Hp, d), dtype=torch.bfloat16, device="cuda") for _ in range(P)] for _ in range(3)]
+    for r in range(P):
+        ws.ulysses_push_seq_to_head(ys, [to_dev(t[r], "bf16") for t in (q_r, k_r, v_r)], Ls, r)
+    zs = [torch.full((Ls + La, H, d), 7.0, dtype=torch.bfloat16, device="cuda") for _ in range(P)]
+    wsp = workspace_for(L, Hp, d, Tc + L)
+    ws.block_causal_attn_push_out(zs, g, Ls, ys[0][g], to_dev(kc, "bf16"), to_dev(vc, "bf16"), Tc, ys[1][g], ys[2][g], qe, kv, scale, wsp)
+    torch.cuda.synchronize()
+    yq, yk, yv = (uly.seq_to_head(t, Ls)[g] for t in (q_r, k_r, v_r))
+    ref, _ = wsref.block_causal_attn(yq, kc, vc, Tc, yk, yv, qe, kv, scale)
+    filler = np.full((L, Hp, d), 7.0, np.float32)
+    want = uly.head_to_seq([ref.astype(np.float32) if i == g else filler for i in range(P)], Ls)
+    for r in range(P):
+        z = to_host(zs[r])
+        assert np.all(np.delete(z, np.s_[g * Hp:(g + 1) * Hp], axis=1) == 7.0), f"rank {r}: other ranks' heads touched"
+        ma, rf = wsref.parity_metrics(z[:, g * Hp:(g + 1) * Hp], want[r][:, g * Hp:(g + 1) * Hp])
+        assert ma <= MAX_ABS and rf <= REL_FRO, f"rank {r}: max_abs={ma:.3e} rel_fro={rf:.3e}"
+
+
 def test_exchange_errors_launch_nothing():
     P, Ls, La, H, d = 2, 8, 2, 4, 64
     x = torch.zeros((Ls + La, H, d), dtype=torch.bfloat16, device="cuda")
