@@ -11,6 +11,8 @@
  *   ws_block_causal_attn   the unit's latent query tokens attend, "coordinated by block-causal
  *                           attention", to the cached K/V conditioning plus the unit's own K/V
  *                                                                   PAPER.md:25, :73, :79
+ *   ws_block_causal_attn_static_ws    a3 for callers that cannot allocate device memory: the scratch is an array
+ *                           inside the library's own device image (at most WS_STATIC_WORKSPACE_BYTES)
  *   ws_block_causal_attn_seq_layout   the two relayouts folded into the attention call (strided TMA)
  *   ws_seq_to_head_multi / ws_head_to_seq_multi   several same-shaped tensors in one launch
  *   ws_kv_cache_write_fp8 / ws_block_causal_attn_fp8kv   the same cache held as FP8 (E4M3 codes and one
@@ -37,7 +39,8 @@
  *     call only.  Device pointers must be 16-byte aligned and d * sizeof(element) a multiple of
  *     16 (WS_ERR_ALIGNMENT otherwise).
  *   - No allocation, no synchronisation, no host read of device data: every call is legal
- *     inside CUDA stream capture.  `stream` is a cudaStream_t passed as void* (NULL = default).
+ *     inside CUDA stream capture (this sentence does not cover ws_block_causal_attn_static_ws, which says
+ *     when its first call on a device must come).  `stream` is a cudaStream_t passed as void* (NULL = default).
  *     Kernels are launched with programmatic stream serialisation (their set-up overlaps the tail
  *     of the previous kernel; they wait for it before touching global memory).
  *   - Batch is 1 (fold a batch into heads).  Layouts are dense row-major with the last index
@@ -73,6 +76,7 @@ typedef enum {
 /* Limits of this build. */
 #define WS_MAX_MASK_BLOCKS 128 /* n_blocks of a ws_block_mask */
 #define WS_MAX_PEERS 8         /* ranks of a Ulysses performer group (ws_ulysses_*, ws_block_causal_attn_push_out) */
+#define WS_STATIC_WORKSPACE_BYTES (64u << 20) /* scratch built into the library for ws_block_causal_attn_static_ws */
 
 /* ------------------------------------------------------------------------------------------------
  * a1. KV cache write
@@ -162,6 +166,41 @@ int ws_block_causal_attn(void* out, float* lse, const void* q, const void* k_cac
                          int64_t capacity, int64_t cache_len, const void* k_new, const void* v_new, int32_t Ln,
                          int32_t H, int32_t d, int32_t Lq, const ws_block_mask* mask, float softmax_scale,
                          void* workspace, size_t workspace_bytes, ws_dtype dt, void* stream);
+
+/* ------------------------------------------------------------------------------------------------
+ * a3 without a caller-supplied workspace: for callers that cannot allocate.
+ *
+ *   ws_block_causal_attn needs scratch in device memory and leaves it to the caller to provide.  Not every caller
+ *   can: a plug-in inside a serving process that handed all of HBM to its framework's pools at start-up (cudaMalloc
+ *   fails, the pool is out of reach from C); the per-unit real-time loop, where a cudaMalloc / cudaFree would
+ *   synchronise the device and stall the units in flight (one unit per 160 ms); code bound by a
+ *   "nothing is allocated after initialisation" rule.  This entry point is ws_block_causal_attn with the scratch
+ *   taken from a fixed array of WS_STATIC_WORKSPACE_BYTES (64 MiB) that is part of the library's device image.  It
+ *   calls no cudaMalloc, cudaFree or any allocating library routine; the caller passes inputs and outputs only.
+ *
+ *   Arguments, arithmetic, results and errors are exactly those of ws_block_causal_attn (the same kernels run on the
+ *   same schedule), minus `workspace` / `workspace_bytes`.
+ *
+ *   Limit:  the problem must satisfy  ws_block_causal_attn_workspace_bytes(Lq, H, d, cache_len + Ln, dt)
+ *           <= WS_STATIC_WORKSPACE_BYTES, else WS_ERR_WORKSPACE is returned and nothing is launched.  64 MiB covers
+ *           every BF16 configuration of BASELINE.json (config 3, 970 x 40 heads x 128: 55.4 MB; the need grows with
+ *           ceil(Lq / 256) * H * d and does not depend on the cache length for BF16 inputs).
+ *   Cost:   every GPU on which the library's device code is loaded holds the 64 MiB until the process exits, used or not.
+ *   First call on a device:  looks up the array's address on that device (cudaGetSymbolAddress, once per device, the
+ *           device being current) and remembers it.  Make that first call during set-up, before any stream capture
+ *           is begun on that device.
+ *   Sharing: every call on a device uses the same array, which still holds whatever the previous call left there.
+ *           No part of it has to be zero on entry -- each call writes what it later reads -- so it is never cleared.
+ *           Two calls that can overlap on the GPU (different streams, or several host threads launching at once)
+ *           race on it and corrupt each other's partial results: keep all calls of a device on one stream, or order
+ *           them with events.  (ws_block_causal_attn with separate workspaces has no such restriction.)
+ *   Errors: as ws_block_causal_attn; WS_ERR_WORKSPACE means "needs more scratch than the built-in array has";
+ *           WS_ERR_CUDA if the address look-up fails.
+ * ---------------------------------------------------------------------------------------------- */
+int ws_block_causal_attn_static_ws(void* out, float* lse, const void* q, const void* k_cache, const void* v_cache,
+                                   int64_t capacity, int64_t cache_len, const void* k_new, const void* v_new, int32_t Ln,
+                                   int32_t H, int32_t d, int32_t Lq, const ws_block_mask* mask, float softmax_scale,
+                                   ws_dtype dt, void* stream);
 
 /* ------------------------------------------------------------------------------------------------
  * a2 + a3 + a4 fused: attention straight on the token-major layout

@@ -9,6 +9,7 @@ from .binding import (  # noqa: F401
     WsError, lib_path, load, version, status_string,
     kv_cache_write, seq_to_head, head_to_seq, seq_to_head_multi, head_to_seq_multi,
     block_causal_attn, block_causal_attn_workspace_bytes, block_causal_attn_seq_layout,
+    block_causal_attn_static_ws, STATIC_WORKSPACE_BYTES,
     kv_cache_write_fp8, block_causal_attn_fp8kv,
     kv_cache_write_ring, block_causal_attn_ring, ring_state,
     ulysses_push_seq_to_head, block_causal_attn_push_out, kv_slice_broadcast_write,

@@ -25,7 +25,9 @@ EXPORTS = (
     "ws_version", "ws_last_cuda_error", "ws_kernel_launch_count", "ws_attn_schedule", "ws_kv_cache_write_fp8", "ws_block_causal_attn_fp8kv",
     "ws_kv_cache_write_ring", "ws_ring_state", "ws_block_causal_attn_ring",
     "ws_ulysses_push_seq_to_head", "ws_block_causal_attn_push_out", "ws_kv_slice_broadcast_write",
+    "ws_block_causal_attn_static_ws",
 )
+STATIC_WORKSPACE_BYTES = 64 << 20  # WS_STATIC_WORKSPACE_BYTES of include/ws.h
 
 
 class WsError(RuntimeError):
@@ -69,6 +71,9 @@ def load():
     lib.ws_block_causal_attn.argtypes = [vp, vp, vp, vp, vp, i64, i64, vp, vp, i32, i32, i32, i32,
                                          ctypes.POINTER(_BlockMask), f32, vp, sz, ctypes.c_int, vp]
     lib.ws_block_causal_attn.restype = ctypes.c_int
+    lib.ws_block_causal_attn_static_ws.argtypes = [vp, vp, vp, vp, vp, i64, i64, vp, vp, i32, i32, i32, i32,
+                                                   ctypes.POINTER(_BlockMask), f32, ctypes.c_int, vp]
+    lib.ws_block_causal_attn_static_ws.restype = ctypes.c_int
     lib.ws_block_causal_attn_seq_layout.argtypes = [vp, vp, vp, vp, vp, i64, i64, vp, vp, i32, i32, i32, i32, i32, i32,
                                                     ctypes.POINTER(_BlockMask), f32, vp, sz, ctypes.c_int, vp]
     lib.ws_block_causal_attn_seq_layout.restype = ctypes.c_int
@@ -251,6 +256,48 @@ def block_causal_attn(out, q, k_cache, v_cache, cache_len: int, k_new, v_new, q_
                                      _p(v_new), Ln, H, d, Lq, ctypes.byref(mask), float(softmax_scale), _p(workspace),
                                      workspace.numel() * workspace.element_size(), _dt(q), _stream(stream))
     _ok(rc, "ws_block_causal_attn")
+
+
+def block_causal_attn_static_ws(out, q, k_cache, v_cache, cache_len: int, k_new, v_new, q_block_end: Sequence[int],
+                                kv_visible: Sequence[int], softmax_scale: float, lse=None, stream=None):
+    """ws_block_causal_attn for callers that cannot allocate device memory (ws.h, ws_block_causal_attn_static_ws).
+
+    Same arguments and results as block_causal_attn, without the workspace: the scratch is a 64 MiB array built into
+    libws.so's device image, so neither this wrapper nor the library allocates anything.  It is meant for code that has
+    no allocator to turn to -- a plug-in in a serving process whose framework owns all of HBM, the per-unit real-time
+    loop where a cudaMalloc would stall the device, set-ups that forbid allocation after start-up.  Problems whose
+    scratch need exceeds STATIC_WORKSPACE_BYTES are refused (WsError, status WS_ERR_WORKSPACE, nothing launched).  All
+    calls on one device share the array: keep them on one stream (overlapping calls race), and make the first call on
+    a device during set-up, before any stream capture."""
+    _dev(out, q, k_cache, v_cache, k_new, v_new, lse)
+    Lq, H, d = q.shape
+    capacity = k_cache.shape[1]
+    Ln = 0 if k_new is None else k_new.shape[0]
+    if out.shape != q.shape or out.dtype != q.dtype:
+        raise ValueError("ws_block_causal_attn_static_ws: out must match q")
+    if tuple(k_cache.shape) != (H, capacity, d) or v_cache.shape != k_cache.shape:
+        raise ValueError("ws_block_causal_attn_static_ws: cache must be [H, capacity, d]")
+    if k_new is not None and (tuple(k_new.shape) != (Ln, H, d) or v_new is None or v_new.shape != k_new.shape):
+        raise ValueError("ws_block_causal_attn_static_ws: k_new/v_new must be [Ln, H, d]")
+    for t in (k_cache, v_cache, k_new, v_new):
+        if t is not None and t.dtype != q.dtype:
+            raise TypeError("ws_block_causal_attn_static_ws: dtype mismatch")
+    if lse is not None and (lse.dtype != torch.float32 or tuple(lse.shape) != (H, Lq)):
+        raise ValueError("ws_block_causal_attn_static_ws: lse must be float32 [H, Lq]")
+    n = len(q_block_end)
+    if len(kv_visible) != n:
+        raise ValueError("ws_block_causal_attn_static_ws: mask arrays differ in length")
+    qe = (ctypes.c_int32 * n)(*[int(x) for x in q_block_end])
+    kv = (ctypes.c_int32 * n)(*[int(x) for x in kv_visible])
+    mask = _BlockMask(n, qe, kv)
+    rc = load().ws_block_causal_attn_static_ws(_p(out), _p(lse), _p(q), _p(k_cache), _p(v_cache), capacity, int(cache_len),
+                                               _p(k_new), _p(v_new), Ln, H, d, Lq, ctypes.byref(mask), float(softmax_scale),
+                                               _dt(q), _stream(stream))
+    if rc == -6:
+        need = block_causal_attn_workspace_bytes(Lq, H, d, int(cache_len) + Ln, q.dtype)
+        raise WsError(rc, f"ws_block_causal_attn_static_ws: this problem needs up to {need} bytes of scratch, the built-in "
+                          f"array holds {STATIC_WORKSPACE_BYTES}")
+    _ok(rc, "ws_block_causal_attn_static_ws")
 
 
 def kv_cache_write_ring(k_cache, v_cache, k_src, v_src, head_begin: int = 0, write_pos: int = 0, stream=None):

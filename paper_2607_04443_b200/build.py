@@ -14,7 +14,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libws.so")
-SOURCES = ["ws_util.cu", "ws_copy.cu", "ws_fp8.cu", "ws_attn.cu", "ws_unit.cu"]
+SOURCES = ["ws_util.cu", "ws_copy.cu", "ws_fp8.cu", "ws_attn.cu", "ws_unit.cu", "ws_static.cu"]
 HEADERS = ["ws_internal.h", "ws_ptx.cuh", os.path.join(ROOT, "include", "ws.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
