@@ -1585,6 +1585,16 @@ extern "C" __attribute__((visibility("default"))) int ws_block_causal_attn_push_
       if (wsi::ranges_overlap(peer_outs[r], peer_bytes, peer_outs[j], peer_bytes)) return WS_ERR_OVERLAP;
     shifted[r] = static_cast<char*>(peer_outs[r]) + off;
   }
+  // A peer's output may not alias anything this call reads or uses as scratch: the epilogue stores finished rows while
+  // other CTAs are still reading Q, K/V and the partial records.  (Sizes of arguments that attn_impl will reject are skipped.)
+  const size_t es = (size_t)wsi::elem_bytes(dt);
+  const size_t new_bytes = Ln > 0 ? (size_t)Ln * H * d * es : 0, cache_bytes = capacity > 0 ? (size_t)H * capacity * d * es : 0;
+  for (int r = 0; r < P; ++r) {
+    const void* reads[] = {q, k_new, v_new, k_cache, v_cache, lse, workspace};
+    const size_t sizes[] = {(size_t)Lq * H * d * es, new_bytes, new_bytes, cache_bytes, cache_bytes, (size_t)H * Lq * 4, workspace_bytes};
+    for (int i = 0; i < 7; ++i)
+      if (reads[i] && wsi::ranges_overlap(peer_outs[r], peer_bytes, reads[i], sizes[i])) return WS_ERR_OVERLAP;
+  }
   return attn_impl(shifted[0], lse, q, k_cache, v_cache, capacity, cache_len, k_new, v_new, Ln, H, d, Lq, mask, softmax_scale, workspace,
                    workspace_bytes, dt, stream, H, nullptr, nullptr, 0, shifted, P, Ls);
 }
@@ -1610,6 +1620,14 @@ extern "C" __attribute__((visibility("default"))) int ws_block_causal_attn_fp8kv
                                           void* stream) {
   if (!k_exp || !v_exp) return WS_ERR_INVALID_ARG;
   if (capacity % 16 != 0 || (reinterpret_cast<uintptr_t>(k_exp) & 15) || (reinterpret_cast<uintptr_t>(v_exp) & 15)) return WS_ERR_ALIGNMENT;
+  // the exponent arrays are read throughout the launch: neither the output nor the scratch may sit on top of them
+  if (out && H > 0 && d > 0 && Lq > 0 && capacity > 0) {
+    const size_t exp_bytes = (size_t)H * capacity, out_bytes = (size_t)Lq * H * d * 2;
+    for (const int8_t* e : {k_exp, v_exp})
+      if (wsi::ranges_overlap(e, exp_bytes, out, out_bytes) || (workspace && wsi::ranges_overlap(e, exp_bytes, workspace, workspace_bytes)) ||
+          (lse && wsi::ranges_overlap(e, exp_bytes, lse, (size_t)H * Lq * 4)))
+        return WS_ERR_OVERLAP;
+  }
   return attn_impl(out, lse, q, k_cache8, v_cache8, capacity, cache_len, k_new, v_new, Ln, H, d, Lq, mask, softmax_scale, workspace,
                    workspace_bytes, WS_DTYPE_BF16, stream, H, k_exp, v_exp);
 }

@@ -215,9 +215,9 @@ def test_ulysses_exchange_entry_points_reject_bad_arguments(lib):
     po = lib.ws_block_causal_attn_push_out
     Mask = binding._BlockMask
 
-    def ocall(outs=(A, B), Pn=2, rank=1, Ls=30, Lq=64, H=2, d=128, q=C):
+    def ocall(outs=(A, B), Pn=2, rank=1, Ls=30, Lq=64, H=2, d=128, q=C, lse=None):
         m = Mask(1, (ctypes.c_int32 * 1)(Lq), (ctypes.c_int32 * 1)(512))
-        return po(arr(*outs), Pn, rank, Ls, None, vp(q), vp(D), vp(0x40000000), 512, 512, None, None, 0, H, d, Lq, ctypes.byref(m), 0.1,
+        return po(arr(*outs), Pn, rank, Ls, vp(lse) if lse else None, vp(q), vp(D), vp(0x40000000), 512, 512, None, None, 0, H, d, Lq, ctypes.byref(m), 0.1,
                   vp(0x70000000), 1 << 30, 0, None)
 
     assert ocall(rank=2) == INVALID
@@ -227,8 +227,35 @@ def test_ulysses_exchange_entry_points_reject_bad_arguments(lib):
     assert ocall(outs=(A, B + 2)) == ALIGN
     assert ocall(d=96) == UNSUPPORTED
     assert ocall(Pn=9, outs=tuple([A] * 9), Ls=7) == UNSUPPORTED
+    # a peer output on top of anything the call reads or uses as scratch (the epilogue would overwrite live data)
+    assert ocall(outs=(A, C + 64)) == OVERLAP           # inside q
+    assert ocall(outs=(C - 64, B)) == OVERLAP           # its tail reaches into q
+    assert ocall(outs=(A, D + 1024)) == OVERLAP         # inside the caches
+    assert ocall(outs=(A, 0x70000000 + 4096)) == OVERLAP  # inside the workspace
+    assert ocall(outs=(A, B), lse=B + 1024) == OVERLAP  # lse inside a peer output
     if not torch.cuda.is_available():
         assert ocall() == CUDA and pcall() == CUDA and bcall() == CUDA     # valid calls reach CUDA: no CPU fallback
+
+
+def test_fp8kv_rejects_exponent_arrays_under_the_output_or_the_scratch(lib):
+    """The per-row exponents of the FP8 cache are read for the whole launch; an output, LSE or workspace laid over them is refused."""
+    f = lib.ws_block_causal_attn_fp8kv
+    Mask = binding._BlockMask
+
+    def call(out=A, lse=None, ke=0x50000000, ve=0x58000000, wsp=0x70000000, cap=512):
+        m = Mask(1, (ctypes.c_int32 * 1)(64), (ctypes.c_int32 * 1)(512))
+        return f(P(out), P(lse) if lse else None, P(B), P(C), P(D), P(ke) if ke else None, P(ve) if ve else None, cap, 512, None, None, 0,
+                 2, 128, 64, ctypes.byref(m), 0.1, P(wsp), 1 << 30, None)
+
+    assert call(ke=0) == INVALID
+    assert call(ke=0x50000004) == ALIGN
+    assert call(cap=520) == ALIGN                      # capacity must be a multiple of 16
+    assert call(ke=A + 256) == OVERLAP                 # K exponents inside the output
+    assert call(ve=A - 512) == OVERLAP                 # V exponents run into the output
+    assert call(ve=0x70000000 + 4096) == OVERLAP       # inside the workspace
+    assert call(lse=0x50000000 + 128) == OVERLAP       # LSE over the K exponents
+    if not torch.cuda.is_available():
+        assert call() == CUDA
 
 
 def test_unit_forward_host_checks_everything_before_enqueueing(lib):

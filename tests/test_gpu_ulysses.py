@@ -245,6 +245,17 @@ def test_exchange_errors_launch_nothing():
     with pytest.raises(ws.WsError) as e:
         ws.block_causal_attn_push_out([zs[0], zs[0]], 0, Ls, q, kc, kc.clone(), 16, None, None, [P * Ls + La], [16], 1.0, wsp)
     assert e.value.status == -5
+    # a peer output laid over the queries, or over the workspace: the epilogue would overwrite what other CTAs still read
+    pool = torch.zeros(8192, dtype=torch.bfloat16, device="cuda")
+    q_in = pool[:q.numel()].view_as(q)
+    z_over_q = pool[1024:1024 + zs[0].numel()].view_as(zs[0])
+    with pytest.raises(ws.WsError) as e:
+        ws.block_causal_attn_push_out([zs[0], z_over_q], 0, Ls, q_in, kc, kc.clone(), 16, None, None, [P * Ls + La], [16], 1.0, wsp)
+    assert e.value.status == -5
+    z_in_wsp = wsp[4096:4096 + 2 * zs[0].numel()].view(torch.bfloat16).view_as(zs[0])
+    with pytest.raises(ws.WsError) as e:
+        ws.block_causal_attn_push_out([z_in_wsp, zs[1]], 0, Ls, q, kc, kc.clone(), 16, None, None, [P * Ls + La], [16], 1.0, wsp)
+    assert e.value.status == -5
     torch.cuda.synchronize()
     assert ws.kernel_launch_count() == n0
     assert all(float((t - 3.0).abs().sum()) == 0.0 for t in ys[0] + zs)
