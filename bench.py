@@ -355,6 +355,33 @@ def cool_down(seconds: float = 0.5):
     time.sleep(seconds)
 
 
+AUX_STAT = ("min of 3 replays of a CUDA graph holding `reps` calls, each measurement started on an idle GPU: a BURST figure, "
+            "not comparable with the headline value or the sustained window, which are means under load")
+
+
+def graph_times(call, reps):
+    """Per-call times (ms, ascending) of three replays of one CUDA graph that holds `reps` calls."""
+    import torch
+    for _ in range(2):
+        call()
+    torch.cuda.synchronize()
+    st, cg = torch.cuda.Stream(), torch.cuda.CUDAGraph()
+    with torch.cuda.graph(cg, stream=st):
+        for _ in range(reps):
+            call()
+    cg.replay()
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ts = []
+    for _ in range(3):
+        a.record()
+        cg.replay()
+        b.record()
+        torch.cuda.synchronize()
+        ts.append(a.elapsed_time(b) / reps)
+    return sorted(ts)
+
+
 def attention_aux(peaks):
     """Attention alone on the other BASELINE.json shapes (device-generated N(0,1) inputs), and the
     config-5 unit (cache write + 8 steps) under one CUDA graph: ms per unit."""
@@ -386,17 +413,17 @@ def attention_aux(peaks):
                 call()
         cg.replay()
         torch.cuda.synchronize()
-        ms = None
+        ts = []
         for _ in range(3):
             a.record()
             cg.replay()
             b.record()
             torch.cuda.synchronize()
-            t = a.elapsed_time(b) / reps
-            ms = t if ms is None else min(ms, t)
+            ts.append(a.elapsed_time(b) / reps)
         del cg
+        ms = min(ts)
         tf = cfg.attn_flops() / ms / 1e9
-        res[name] = {"attention_ms": ms, "tflops": tf, "frac_bf16_peak": tf / peaks["bf16_tflops"]}
+        res[name] = {"attention_ms": ms, "attention_ms_median": sorted(ts)[1], "tflops": tf, "frac_bf16_peak": tf / peaks["bf16_tflops"]}
         if name == "cfg4":
             # one Ulysses rank's local step (P = 4): seq->head x3 + attention + head->seq, against the same step
             # with the relayouts fused into the attention call (strided TMA on the token-major tensors)
@@ -454,6 +481,7 @@ def attention_aux(peaks):
                                       "frac_of_sustained_peak": tf / peaks["bf16_tflops_sustained"],
                                       "paper_budget_ms_per_unit_all_layers": 160.0}
         del kc, vc
+    res["stat"] = AUX_STAT + "; cfg4_rank_step_* and cfg5_unit_graph are plain means (10 eager calls / 3 graph replays)"
     return res
 
 
@@ -466,26 +494,7 @@ def fp8_aux(peaks):
     g = torch.Generator(device="cuda").manual_seed(8)
     rnd = lambda std, *s: (torch.randn(*s, generator=g, device="cuda", dtype=torch.float32) * std).to(torch.bfloat16)
 
-    def graph_ms(call, reps):
-        for _ in range(2):
-            call()
-        torch.cuda.synchronize()
-        st, cg = torch.cuda.Stream(), torch.cuda.CUDAGraph()
-        with torch.cuda.graph(cg, stream=st):
-            for _ in range(reps):
-                call()
-        cg.replay()
-        torch.cuda.synchronize()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        best = None
-        for _ in range(3):
-            a.record()
-            cg.replay()
-            b.record()
-            torch.cuda.synchronize()
-            t = a.elapsed_time(b) / reps
-            best = t if best is None else min(best, t)
-        return best
+    graph_ms = lambda call, reps: graph_times(call, reps)[0]
 
     for name in ("cfg2", "cfg3", "cfg5"):
         cool_down()
@@ -499,10 +508,11 @@ def fp8_aux(peaks):
         q, kn, vn = rnd(cfg.q_premul, L, H, d), rnd(cfg.kv_std, L, H, d), rnd(cfg.kv_std, L, H, d)
         out = torch.empty_like(q)
         wsp = torch.empty(ws.block_causal_attn_workspace_bytes(L, H, d, Tc + cfg.Ln), dtype=torch.uint8, device="cuda")
-        ms = graph_ms(lambda: ws.block_causal_attn_fp8kv(out, q, kc8, vc8, ke, ve, Tc, kn, vn, cfg.q_block_end, cfg.kv_visible,
-                                                         cfg.softmax_scale, wsp), 10)
+        ts = graph_times(lambda: ws.block_causal_attn_fp8kv(out, q, kc8, vc8, ke, ve, Tc, kn, vn, cfg.q_block_end, cfg.kv_visible,
+                                                            cfg.softmax_scale, wsp), 10)
+        ms = ts[0]
         tf = cfg.attn_flops() / ms / 1e9
-        res[name] = {"attention_ms_fp8_cache": ms, "tflops": tf, "frac_bf16_peak": tf / peaks["bf16_tflops"],
+        res[name] = {"attention_ms_fp8_cache": ms, "attention_ms_fp8_cache_median": ts[1], "tflops": tf, "frac_bf16_peak": tf / peaks["bf16_tflops"],
                      "cache_bytes_fp8": 2 * H * cap * (d + 1), "cache_bytes_bf16": 2 * H * cap * d * 2}
         del kc8, vc8, ke, ve
     # cache write at cfg3's slice size, rotating over 64 windows of a 65536-row cache and 24 source sets
@@ -529,6 +539,7 @@ def fp8_aux(peaks):
     ms = graph_ms(wr2, 16)
     byts = 2 * 8192 * H * (2 * d + d + 1)
     res["cache_write_fp8_8192rows"] = {"us": ms * 1e3, "gbs": byts / ms / 1e6, "bytes": byts, "frac_hbm": byts / ms / 1e6 / peaks["hbm_gbs"]}
+    res["stat"] = AUX_STAT
     return res
 
 
@@ -542,26 +553,7 @@ def next_rows_aux(peaks):
     g = torch.Generator(device="cuda").manual_seed(9)
     rnd = lambda std, *s: (torch.randn(*s, generator=g, device="cuda", dtype=torch.float32) * std).to(torch.bfloat16)
 
-    def graph_ms(call, reps=10):
-        for _ in range(2):
-            call()
-        torch.cuda.synchronize()
-        st, cg = torch.cuda.Stream(), torch.cuda.CUDAGraph()
-        with torch.cuda.graph(cg, stream=st):
-            for _ in range(reps):
-                call()
-        cg.replay()
-        torch.cuda.synchronize()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        best = None
-        for _ in range(3):
-            a.record()
-            cg.replay()
-            b.record()
-            torch.cuda.synchronize()
-            t = a.elapsed_time(b) / reps
-            best = t if best is None else min(best, t)
-        return best
+    graph_ms = lambda call, reps=10: graph_times(call, reps)[0]
 
     # ---- ring cache: cfg3 shape, the ring exactly as large as the window (16384 rows), 23 units of 970 rows written
     cfg = wl.CONFIGS["cfg3"]
@@ -610,6 +602,7 @@ def next_rows_aux(peaks):
     ms_b = graph_ms(lambda: ws.kv_slice_broadcast_write(kcs, vcs, ks, vs, 15360), 50)
     byts = 2 * 2 * 1024 * Ht * d * 2
     res["kv_slice_broadcast_write_4ranks"] = {"us": ms_b * 1e3, "bytes": byts, "gbs_l2_resident": byts / ms_b / 1e6, "launches": 1}
+    res["stat"] = AUX_STAT
     return res
 
 
