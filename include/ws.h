@@ -58,7 +58,9 @@
 extern "C" {
 #endif
 
-#define WS_VERSION 100 /* major*10000 + minor*100 + patch */
+/* major*10000 + minor*100 + patch.  0.1.0: rows a1-a5.  0.2.0: ws_attn_schedule gained unit_kv_tiles (NOT call-compatible
+ * with 0.1.0), FP8 / ring / Ulysses entry points.  0.3.0: ws_block_causal_attn_static_ws, overlap rules of push_out / fp8kv. */
+#define WS_VERSION 300
 
 typedef enum { WS_DTYPE_BF16 = 0, WS_DTYPE_F32 = 1 } ws_dtype;
 

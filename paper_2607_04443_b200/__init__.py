@@ -14,5 +14,5 @@ from .binding import (  # noqa: F401
     kv_cache_write_ring, block_causal_attn_ring, ring_state,
     ulysses_push_seq_to_head, block_causal_attn_push_out, kv_slice_broadcast_write,
     unit_forward_host, unit_forward_host_staging_bytes, kernel_launch_count, attn_schedule, EXPORTS,
-    DTYPE_BF16, DTYPE_F32,
+    DTYPE_BF16, DTYPE_F32, ABI_VERSION,
 )

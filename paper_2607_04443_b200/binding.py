@@ -14,6 +14,7 @@ import torch
 
 DTYPE_BF16 = 0
 DTYPE_F32 = 1
+ABI_VERSION = 300  # WS_VERSION of include/ws.h this binding was written against
 
 _PKG = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_PKG, "libws.so")
@@ -109,6 +110,9 @@ def load():
     for fn in (lib.ws_version, lib.ws_last_cuda_error, lib.ws_kernel_launch_count):
         fn.argtypes = []
         fn.restype = ctypes.c_int
+    if int(lib.ws_version()) != ABI_VERSION:  # a stale build would be called with the wrong argument lists
+        raise RuntimeError(f"{_LIB_PATH} reports version {int(lib.ws_version())}, this binding needs {ABI_VERSION}: rebuild it with "
+                           "`python -m paper_2607_04443_b200.build --force`")
     _lib = lib
     return lib
 

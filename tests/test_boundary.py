@@ -41,7 +41,7 @@ def test_library_exports_every_declared_symbol(lib):
 
 
 def test_version_and_status_strings(lib):
-    assert ws.version() == 100
+    assert ws.version() == ws.ABI_VERSION == 300
     assert ws.status_string(0) == "WS_OK"
     for code in range(-7, 0):
         assert ws.status_string(code).startswith("WS_ERR_")
