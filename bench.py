@@ -628,6 +628,27 @@ def run_fp8_kernels_only(args):
     print("fp8 kernels ok")
 
 
+def run_attn_only(args):
+    """ws_block_causal_attn alone on one BASELINE.json shape (device-generated inputs as in attention_aux), for ncu:
+    args.warmup + args.steps calls, no JSON line."""
+    import torch
+    import paper_2607_04443_b200 as ws
+    cfg = wl.CONFIGS[args.attn_only]
+    g = torch.Generator(device="cuda").manual_seed(6)
+    rnd = lambda std, *s: (torch.randn(*s, generator=g, device="cuda", dtype=torch.float32) * std).to(torch.bfloat16)
+    L, H, d = cfg.Lq, cfg.H, cfg.d
+    kc, vc = rnd(cfg.kv_std, H, cfg.capacity, d), rnd(cfg.kv_std, H, cfg.capacity, d)
+    q, kn, vn = rnd(cfg.q_premul, L, H, d), rnd(cfg.kv_std, L, H, d), rnd(cfg.kv_std, L, H, d)
+    out = torch.empty_like(q)
+    wsp = torch.empty(ws.block_causal_attn_workspace_bytes(L, H, d, cfg.cache_len + cfg.Ln), dtype=torch.uint8, device="cuda")
+    n0 = ws.kernel_launch_count()
+    for _ in range(args.warmup + args.steps):
+        ws.block_causal_attn(out, q, kc, vc, cfg.cache_len, kn, vn, cfg.q_block_end, cfg.kv_visible, cfg.softmax_scale, wsp)
+    torch.cuda.synchronize()
+    assert torch.isfinite(out.float()).all()
+    print(f"attention on {cfg.name} ok: {(ws.kernel_launch_count() - n0) // (args.warmup + args.steps)} launches per call")
+
+
 def cpu_oracle_sample(cfg, x, target_seconds: float = 12.0):
     """The oracle as it stands on a bounded sample of (row, head) pairs of this workload."""
     from oracle import wsref
@@ -831,9 +852,13 @@ def main():
                     help="profiling mode: only the device-resident timed steps (no e2e, cpu_baseline or aux legs)")
     ap.add_argument("--fp8-kernels-only", action="store_true",
                     help="profiling mode: cfg3 with the cache held as FP8 (ws_kv_cache_write_fp8 + ws_block_causal_attn_fp8kv), a few calls, no JSON line")
+    ap.add_argument("--attn-only", choices=["cfg2", "cfg3", "cfg4", "cfg5"], default=None,
+                    help="profiling mode: ws_block_causal_attn alone on that BASELINE.json shape, a few calls, no JSON line")
     args = ap.parse_args()
     if args.fp8_kernels_only:
         return run_fp8_kernels_only(args)
+    if args.attn_only:
+        return run_attn_only(args)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)

@@ -250,6 +250,10 @@ int ws_block_causal_attn_seq_layout(void* out_seq, float* lse, const void* q_seq
  *   ws_block_causal_attn_fp8kv:  a3 with that cache; q, k_new, v_new, out stay BF16 [L, H, d].  The codes are
  *   expanded to BF16 inside the SM (exactly), so the result is what ws_block_causal_attn returns on the dequantised
  *   cache, up to the order of FP32 summation.  Workspace size as ws_block_causal_attn (WS_DTYPE_BF16).
+ *   Sources must be FINITE.  A NaN element is stored as the E4M3 NaN code (0x7f / 0xff) and leaves the exponent and codes of
+ *   its own (row, head) group unspecified (other groups are unaffected); ws_block_causal_attn_fp8kv does not decode NaN codes
+ *   as NaN but as the finite value +-480 * 2^e, so a NaN written into the FP8 cache does NOT surface in the output the way it
+ *   does with the BF16 cache.  +-Inf saturates to +-448 * 2^7.  (Pinned by tests/test_gpu_fp8.py.)
  *   Both: d in {64, 128}; capacity a multiple of 16 and every pointer 16-byte aligned (ALIGNMENT otherwise); the
  *   other errors as their BF16 counterparts.
  * ---------------------------------------------------------------------------------------------- */
@@ -351,7 +355,7 @@ int ws_kv_slice_broadcast_write(void* const* peer_k_caches, void* const* peer_v_
  *   attention of a step is split by key source: Q[s] against the CACHE starts as soon as the slice and Q[s] have landed
  *   and runs under the transfer of the unit's own K/V; Q[s] against the unit's own rows follows, and a small kernel
  *   merges the two (attention over a union of key sets = LSE-weighted mean of the two attentions; both partial results
- *   are BF16, so the merged output carries one more BF16 rounding than ws_block_causal_attn's).  Outputs return on a
+ *   stay FP32 until they are merged, so the output is rounded to BF16 once, like ws_block_causal_attn's).  Outputs return on a
  *   second internal stream.  Both helper streams (one pair per device, created on first use: the library's only lazily
  *   created global state besides the driver entry point) start after the work already queued on `stream` and are
  *   joined back into it -- also when a CUDA call fails half way -- so to the caller the call is ordered on `stream`

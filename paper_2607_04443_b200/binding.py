@@ -232,30 +232,41 @@ def block_causal_attn_workspace_bytes(Lq: int, H: int, d: int, kv_total: int, dt
     return int(load().ws_block_causal_attn_workspace_bytes(Lq, H, d, kv_total, dt))
 
 
+def _attn_args(name, out, q, k_cache, v_cache, k_new, v_new, lse, q_block_end, kv_visible, token_major=False, cache_dtype=None):
+    """The shape, dtype and mask rules shared by every attention wrapper.  q (and out, k_new, v_new) are [L, Hq, d]; the cache
+    is [H, capacity, d] with H == Hq, except for the token-major call (token_major=True) where the cache names the H of the
+    Hq heads that take part.  cache_dtype overrides the cache's element type (uint8 codes for the FP8 cache).
+    Returns (Lq, H, d, capacity, Ln, mask); `mask` keeps its arrays alive."""
+    Lq, Hq, d = q.shape
+    capacity = k_cache.shape[1]
+    H = k_cache.shape[0] if token_major else Hq
+    Ln = 0 if k_new is None else k_new.shape[0]
+    if out is not None and (out.shape != q.shape or out.dtype != q.dtype):
+        raise ValueError(f"{name}: out must match q")
+    if tuple(k_cache.shape) != (H, capacity, d) or v_cache.shape != k_cache.shape:
+        raise ValueError(f"{name}: cache must be [H, capacity, d]")
+    if k_new is not None and (tuple(k_new.shape) != (Ln, Hq, d) or v_new is None or v_new.shape != k_new.shape):
+        raise ValueError(f"{name}: k_new/v_new must be [Ln, {'H_total' if token_major else 'H'}, d]")
+    for t, want in ((k_cache, cache_dtype or q.dtype), (v_cache, cache_dtype or q.dtype), (k_new, q.dtype), (v_new, q.dtype)):
+        if t is not None and t.dtype != want:
+            raise TypeError(f"{name}: dtype mismatch")
+    if lse is not None and (lse.dtype != torch.float32 or tuple(lse.shape) != (H, Lq)):
+        raise ValueError(f"{name}: lse must be float32 [H, Lq]")
+    n = len(q_block_end)
+    if len(kv_visible) != n:
+        raise ValueError(f"{name}: mask arrays differ in length")
+    qe = (ctypes.c_int32 * n)(*[int(x) for x in q_block_end])
+    kv = (ctypes.c_int32 * n)(*[int(x) for x in kv_visible])
+    mask = _BlockMask(n, qe, kv)
+    mask._keep = (qe, kv)
+    return Lq, H, d, capacity, Ln, mask
+
+
 def block_causal_attn(out, q, k_cache, v_cache, cache_len: int, k_new, v_new, q_block_end: Sequence[int],
                       kv_visible: Sequence[int], softmax_scale: float, workspace, lse=None, stream=None):
     """Block-causal unit attention (ws.h a3).  out/q [Lq,H,d]; caches [H,capacity,d]; k_new/v_new [Ln,H,d] or None."""
     _dev(out, q, k_cache, v_cache, k_new, v_new, workspace, lse)
-    Lq, H, d = q.shape
-    capacity = k_cache.shape[1]
-    Ln = 0 if k_new is None else k_new.shape[0]
-    if out.shape != q.shape or out.dtype != q.dtype:
-        raise ValueError("ws_block_causal_attn: out must match q")
-    if tuple(k_cache.shape) != (H, capacity, d) or v_cache.shape != k_cache.shape:
-        raise ValueError("ws_block_causal_attn: cache must be [H, capacity, d]")
-    if k_new is not None and (tuple(k_new.shape) != (Ln, H, d) or v_new is None or v_new.shape != k_new.shape):
-        raise ValueError("ws_block_causal_attn: k_new/v_new must be [Ln, H, d]")
-    for t in (k_cache, v_cache, k_new, v_new):
-        if t is not None and t.dtype != q.dtype:
-            raise TypeError("ws_block_causal_attn: dtype mismatch")
-    if lse is not None and (lse.dtype != torch.float32 or tuple(lse.shape) != (H, Lq)):
-        raise ValueError("ws_block_causal_attn: lse must be float32 [H, Lq]")
-    n = len(q_block_end)
-    if len(kv_visible) != n:
-        raise ValueError("ws_block_causal_attn: mask arrays differ in length")
-    qe = (ctypes.c_int32 * n)(*[int(x) for x in q_block_end])
-    kv = (ctypes.c_int32 * n)(*[int(x) for x in kv_visible])
-    mask = _BlockMask(n, qe, kv)
+    Lq, H, d, capacity, Ln, mask = _attn_args("ws_block_causal_attn", out, q, k_cache, v_cache, k_new, v_new, lse, q_block_end, kv_visible)
     rc = load().ws_block_causal_attn(_p(out), _p(lse), _p(q), _p(k_cache), _p(v_cache), capacity, int(cache_len), _p(k_new),
                                      _p(v_new), Ln, H, d, Lq, ctypes.byref(mask), float(softmax_scale), _p(workspace),
                                      workspace.numel() * workspace.element_size(), _dt(q), _stream(stream))
@@ -274,26 +285,7 @@ def block_causal_attn_static_ws(out, q, k_cache, v_cache, cache_len: int, k_new,
     calls on one device share the array: keep them on one stream (overlapping calls race), and make the first call on
     a device during set-up, before any stream capture."""
     _dev(out, q, k_cache, v_cache, k_new, v_new, lse)
-    Lq, H, d = q.shape
-    capacity = k_cache.shape[1]
-    Ln = 0 if k_new is None else k_new.shape[0]
-    if out.shape != q.shape or out.dtype != q.dtype:
-        raise ValueError("ws_block_causal_attn_static_ws: out must match q")
-    if tuple(k_cache.shape) != (H, capacity, d) or v_cache.shape != k_cache.shape:
-        raise ValueError("ws_block_causal_attn_static_ws: cache must be [H, capacity, d]")
-    if k_new is not None and (tuple(k_new.shape) != (Ln, H, d) or v_new is None or v_new.shape != k_new.shape):
-        raise ValueError("ws_block_causal_attn_static_ws: k_new/v_new must be [Ln, H, d]")
-    for t in (k_cache, v_cache, k_new, v_new):
-        if t is not None and t.dtype != q.dtype:
-            raise TypeError("ws_block_causal_attn_static_ws: dtype mismatch")
-    if lse is not None and (lse.dtype != torch.float32 or tuple(lse.shape) != (H, Lq)):
-        raise ValueError("ws_block_causal_attn_static_ws: lse must be float32 [H, Lq]")
-    n = len(q_block_end)
-    if len(kv_visible) != n:
-        raise ValueError("ws_block_causal_attn_static_ws: mask arrays differ in length")
-    qe = (ctypes.c_int32 * n)(*[int(x) for x in q_block_end])
-    kv = (ctypes.c_int32 * n)(*[int(x) for x in kv_visible])
-    mask = _BlockMask(n, qe, kv)
+    Lq, H, d, capacity, Ln, mask = _attn_args("ws_block_causal_attn_static_ws", out, q, k_cache, v_cache, k_new, v_new, lse, q_block_end, kv_visible)
     rc = load().ws_block_causal_attn_static_ws(_p(out), _p(lse), _p(q), _p(k_cache), _p(v_cache), capacity, int(cache_len),
                                                _p(k_new), _p(v_new), Ln, H, d, Lq, ctypes.byref(mask), float(softmax_scale),
                                                _dt(q), _stream(stream))
@@ -330,26 +322,7 @@ def block_causal_attn_ring(out, q, k_cache, v_cache, ring_start: int, cache_len:
     """Block-causal unit attention on a ring cache (ws.h ws_block_causal_attn_ring): cache key j is physical row
     (ring_start + j) mod capacity.  Shapes as block_causal_attn."""
     _dev(out, q, k_cache, v_cache, k_new, v_new, workspace, lse)
-    Lq, H, d = q.shape
-    capacity = k_cache.shape[1]
-    Ln = 0 if k_new is None else k_new.shape[0]
-    if out.shape != q.shape or out.dtype != q.dtype:
-        raise ValueError("ws_block_causal_attn_ring: out must match q")
-    if tuple(k_cache.shape) != (H, capacity, d) or v_cache.shape != k_cache.shape:
-        raise ValueError("ws_block_causal_attn_ring: cache must be [H, capacity, d]")
-    if k_new is not None and (tuple(k_new.shape) != (Ln, H, d) or v_new is None or v_new.shape != k_new.shape):
-        raise ValueError("ws_block_causal_attn_ring: k_new/v_new must be [Ln, H, d]")
-    for t in (k_cache, v_cache, k_new, v_new):
-        if t is not None and t.dtype != q.dtype:
-            raise TypeError("ws_block_causal_attn_ring: dtype mismatch")
-    if lse is not None and (lse.dtype != torch.float32 or tuple(lse.shape) != (H, Lq)):
-        raise ValueError("ws_block_causal_attn_ring: lse must be float32 [H, Lq]")
-    n = len(q_block_end)
-    if len(kv_visible) != n:
-        raise ValueError("ws_block_causal_attn_ring: mask arrays differ in length")
-    qe = (ctypes.c_int32 * n)(*[int(x) for x in q_block_end])
-    kv = (ctypes.c_int32 * n)(*[int(x) for x in kv_visible])
-    mask = _BlockMask(n, qe, kv)
+    Lq, H, d, capacity, Ln, mask = _attn_args("ws_block_causal_attn_ring", out, q, k_cache, v_cache, k_new, v_new, lse, q_block_end, kv_visible)
     rc = load().ws_block_causal_attn_ring(_p(out), _p(lse), _p(q), _p(k_cache), _p(v_cache), capacity, int(ring_start), int(cache_len),
                                           _p(k_new), _p(v_new), Ln, H, d, Lq, ctypes.byref(mask), float(softmax_scale), _p(workspace),
                                           workspace.numel() * workspace.element_size(), _dt(q), _stream(stream))
@@ -392,28 +365,12 @@ def block_causal_attn_push_out(peer_outs, rank: int, Ls: int, q, k_cache, v_cach
     peer_outs = list(peer_outs)
     _dev(*peer_outs, q, k_cache, v_cache, k_new, v_new, workspace, lse)
     P = len(peer_outs)
-    Lq, H, d = q.shape
-    capacity = k_cache.shape[1]
-    Ln = 0 if k_new is None else k_new.shape[0]
+    Lq, H, d, capacity, Ln, mask = _attn_args("ws_block_causal_attn_push_out", None, q, k_cache, v_cache, k_new, v_new, lse,
+                                              q_block_end, kv_visible)
     La = Lq - P * Ls
     for z in peer_outs:
         if z.dtype != q.dtype or tuple(z.shape) != (Ls + La, P * H, d):
             raise ValueError("ws_block_causal_attn_push_out: peer outputs must be [Ls + La, P * H, d]")
-    if tuple(k_cache.shape) != (H, capacity, d) or v_cache.shape != k_cache.shape:
-        raise ValueError("ws_block_causal_attn_push_out: cache must be [H, capacity, d]")
-    if k_new is not None and (tuple(k_new.shape) != (Ln, H, d) or v_new is None or v_new.shape != k_new.shape):
-        raise ValueError("ws_block_causal_attn_push_out: k_new/v_new must be [Ln, H, d]")
-    for t in (k_cache, v_cache, k_new, v_new):
-        if t is not None and t.dtype != q.dtype:
-            raise TypeError("ws_block_causal_attn_push_out: dtype mismatch")
-    if lse is not None and (lse.dtype != torch.float32 or tuple(lse.shape) != (H, Lq)):
-        raise ValueError("ws_block_causal_attn_push_out: lse must be float32 [H, Lq]")
-    n = len(q_block_end)
-    if len(kv_visible) != n:
-        raise ValueError("ws_block_causal_attn_push_out: mask arrays differ in length")
-    qe = (ctypes.c_int32 * n)(*[int(x) for x in q_block_end])
-    kv = (ctypes.c_int32 * n)(*[int(x) for x in kv_visible])
-    mask = _BlockMask(n, qe, kv)
     rc = load().ws_block_causal_attn_push_out(_ptr_array(peer_outs), P, int(rank), int(Ls), _p(lse), _p(q), _p(k_cache), _p(v_cache),
                                               capacity, int(cache_len), _p(k_new), _p(v_new), Ln, H, d, Lq, ctypes.byref(mask),
                                               float(softmax_scale), _p(workspace), workspace.numel() * workspace.element_size(),
@@ -459,26 +416,12 @@ def block_causal_attn_fp8kv(out, q, k_cache8, v_cache8, k_exp, v_exp, cache_len:
                             kv_visible: Sequence[int], softmax_scale: float, workspace, lse=None, stream=None):
     """Block-causal unit attention on an FP8 cache (ws.h ws_block_causal_attn_fp8kv); q/out/k_new/v_new BF16."""
     _dev(out, q, k_cache8, v_cache8, k_exp, v_exp, k_new, v_new, workspace, lse)
-    Lq, H, d = q.shape
-    capacity = k_cache8.shape[1]
-    Ln = 0 if k_new is None else k_new.shape[0]
-    if out.shape != q.shape or out.dtype != q.dtype or q.dtype != torch.bfloat16:
-        raise ValueError("ws_block_causal_attn_fp8kv: out must match q (bfloat16)")
-    if tuple(k_cache8.shape) != (H, capacity, d) or v_cache8.shape != k_cache8.shape or tuple(k_exp.shape) != (H, capacity) or \
-            v_exp.shape != k_exp.shape or k_cache8.dtype != torch.uint8 or v_cache8.dtype != torch.uint8 or \
-            k_exp.dtype != torch.int8 or v_exp.dtype != torch.int8:
-        raise ValueError("ws_block_causal_attn_fp8kv: cache uint8 [H, capacity, d], exponents int8 [H, capacity]")
-    if k_new is not None and (tuple(k_new.shape) != (Ln, H, d) or v_new is None or v_new.shape != k_new.shape or
-                              k_new.dtype != q.dtype or v_new.dtype != q.dtype):
-        raise ValueError("ws_block_causal_attn_fp8kv: k_new/v_new must be bfloat16 [Ln, H, d]")
-    if lse is not None and (lse.dtype != torch.float32 or tuple(lse.shape) != (H, Lq)):
-        raise ValueError("ws_block_causal_attn_fp8kv: lse must be float32 [H, Lq]")
-    n = len(q_block_end)
-    if len(kv_visible) != n:
-        raise ValueError("ws_block_causal_attn_fp8kv: mask arrays differ in length")
-    qe = (ctypes.c_int32 * n)(*[int(x) for x in q_block_end])
-    kv = (ctypes.c_int32 * n)(*[int(x) for x in kv_visible])
-    mask = _BlockMask(n, qe, kv)
+    if q.dtype != torch.bfloat16:
+        raise TypeError("ws_block_causal_attn_fp8kv: q, out, k_new, v_new must be bfloat16")
+    Lq, H, d, capacity, Ln, mask = _attn_args("ws_block_causal_attn_fp8kv", out, q, k_cache8, v_cache8, k_new, v_new, lse,
+                                              q_block_end, kv_visible, cache_dtype=torch.uint8)
+    if tuple(k_exp.shape) != (H, capacity) or v_exp.shape != k_exp.shape or k_exp.dtype != torch.int8 or v_exp.dtype != torch.int8:
+        raise ValueError("ws_block_causal_attn_fp8kv: exponents must be int8 [H, capacity]")
     rc = load().ws_block_causal_attn_fp8kv(_p(out), _p(lse), _p(q), _p(k_cache8), _p(v_cache8), _p(k_exp), _p(v_exp), capacity,
                                            int(cache_len), _p(k_new), _p(v_new), Ln, H, d, Lq, ctypes.byref(mask), float(softmax_scale),
                                            _p(workspace), workspace.numel() * workspace.element_size(), _stream(stream))
@@ -491,26 +434,9 @@ def block_causal_attn_seq_layout(out_seq, q_seq, k_cache, v_cache, cache_len: in
     """Relayouts fused into attention (ws.h a2+a3+a4): q_seq/out_seq [Lq, H_total, d], k_new_seq/v_new_seq
     [Ln, H_total, d] or None; the cache [H, capacity, d] names the H heads [head_begin, head_begin + H) taken."""
     _dev(out_seq, q_seq, k_cache, v_cache, k_new_seq, v_new_seq, workspace, lse)
-    Lq, H_total, d = q_seq.shape
-    H, capacity = k_cache.shape[0], k_cache.shape[1]
-    Ln = 0 if k_new_seq is None else k_new_seq.shape[0]
-    if out_seq.shape != q_seq.shape or out_seq.dtype != q_seq.dtype:
-        raise ValueError("ws_block_causal_attn_seq_layout: out_seq must match q_seq")
-    if tuple(k_cache.shape) != (H, capacity, d) or v_cache.shape != k_cache.shape:
-        raise ValueError("ws_block_causal_attn_seq_layout: cache must be [H, capacity, d]")
-    if k_new_seq is not None and (tuple(k_new_seq.shape) != (Ln, H_total, d) or v_new_seq is None or v_new_seq.shape != k_new_seq.shape):
-        raise ValueError("ws_block_causal_attn_seq_layout: k_new_seq/v_new_seq must be [Ln, H_total, d]")
-    for t in (k_cache, v_cache, k_new_seq, v_new_seq):
-        if t is not None and t.dtype != q_seq.dtype:
-            raise TypeError("ws_block_causal_attn_seq_layout: dtype mismatch")
-    if lse is not None and (lse.dtype != torch.float32 or tuple(lse.shape) != (H, Lq)):
-        raise ValueError("ws_block_causal_attn_seq_layout: lse must be float32 [H, Lq]")
-    n = len(q_block_end)
-    if len(kv_visible) != n:
-        raise ValueError("ws_block_causal_attn_seq_layout: mask arrays differ in length")
-    qe = (ctypes.c_int32 * n)(*[int(x) for x in q_block_end])
-    kv = (ctypes.c_int32 * n)(*[int(x) for x in kv_visible])
-    mask = _BlockMask(n, qe, kv)
+    H_total = q_seq.shape[1]
+    Lq, H, d, capacity, Ln, mask = _attn_args("ws_block_causal_attn_seq_layout", out_seq, q_seq, k_cache, v_cache, k_new_seq, v_new_seq,
+                                              lse, q_block_end, kv_visible, token_major=True)
     rc = load().ws_block_causal_attn_seq_layout(_p(out_seq), _p(lse), _p(q_seq), _p(k_cache), _p(v_cache), capacity, int(cache_len),
                                                 _p(k_new_seq), _p(v_new_seq), Ln, H_total, int(head_begin), H, d, Lq,
                                                 ctypes.byref(mask), float(softmax_scale), _p(workspace),

@@ -1423,7 +1423,7 @@ int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const v
               int64_t cache_len, const void* k_new, const void* v_new, int32_t Ln, int32_t H, int32_t d, int32_t Lq,
               const ws_block_mask* mask, float softmax_scale, void* workspace, size_t workspace_bytes, ws_dtype dt,
               void* stream_, int64_t tok_heads, const int8_t* k_exp = nullptr, const int8_t* v_exp = nullptr, int64_t ring_start = 0,
-              void* const* peer_outs = nullptr, int32_t n_peers = 1, int64_t peer_rows = 0) {
+              void* const* peer_outs = nullptr, int32_t n_peers = 1, int64_t peer_rows = 0, bool f32_out_only = false) {
   cudaStream_t stream = (cudaStream_t)stream_;
   const bool kv8 = k_exp != nullptr;  // the cache holds E4M3 codes with per-row exponents (ws_block_causal_attn_fp8kv)
   // ---- validation, descriptors and schedule first: nothing is launched on any error ----
@@ -1531,6 +1531,8 @@ int attn_impl(void* out, float* lse, const void* q, const void* k_cache, const v
     if (ce != cudaSuccess) return wsi::cuda_fail(ce);
   }
   if (kv8) return d == 128 ? launch_attention<128, false, true>(prm, dev, stream) : launch_attention<64, false, true>(prm, dev, stream);
+  // BF16 operands read in place, FP32 rows out (wsi::attn_bf16_in_f32_out): the FP32 epilogue without the staging casts
+  if (f32_out_only) return d == 128 ? launch_attention<128, true, false>(prm, dev, stream) : launch_attention<64, true, false>(prm, dev, stream);
   if (d == 128) return f32 ? launch_attention<128, true, false>(prm, dev, stream) : launch_attention<128, false, false>(prm, dev, stream);
   return f32 ? launch_attention<64, true, false>(prm, dev, stream) : launch_attention<64, false, false>(prm, dev, stream);
 }
@@ -1542,6 +1544,15 @@ extern "C" __attribute__((visibility("default"))) int ws_block_causal_attn(void*
                                     void* workspace, size_t workspace_bytes, ws_dtype dt, void* stream) {
   return attn_impl(out, lse, q, k_cache, v_cache, capacity, cache_len, k_new, v_new, Ln, H, d, Lq, mask, softmax_scale, workspace,
                    workspace_bytes, dt, stream, H);
+}
+
+// Internal (ws_unit.cu): ws_block_causal_attn on BF16 inputs whose output rows are written as FP32 [Lq, H, d] -- the
+// normalised O before its rounding to BF16, for partial results that are merged afterwards.
+int wsi::attn_bf16_in_f32_out(float* out, float* lse, const void* q, const void* k_cache, const void* v_cache, int64_t capacity,
+                              int64_t cache_len, const void* k_new, const void* v_new, int32_t Ln, int32_t H, int32_t d, int32_t Lq,
+                              const ws_block_mask* mask, float softmax_scale, void* workspace, size_t workspace_bytes, void* stream) {
+  return attn_impl(out, lse, q, k_cache, v_cache, capacity, cache_len, k_new, v_new, Ln, H, d, Lq, mask, softmax_scale, workspace,
+                   workspace_bytes, WS_DTYPE_BF16, stream, H, nullptr, nullptr, 0, nullptr, 1, 0, true);
 }
 
 // a2 + a3 + a4 in one call: the rank's heads [head_begin, head_begin + H) are read straight from

@@ -26,6 +26,11 @@ inline bool ranges_overlap(const void* a, size_t na, const void* b, size_t nb) {
 int attn_validate(const void* out, const float* lse, const void* q, const void* k_cache, const void* v_cache, int64_t capacity,
                   int64_t cache_len, const void* k_new, const void* v_new, int32_t Ln, int32_t H, int32_t d, int32_t Lq,
                   const ws_block_mask* mask, float softmax_scale, const void* workspace, size_t workspace_bytes, ws_dtype dt);
+// ws_block_causal_attn on BF16 inputs with the output rows written as FP32 [Lq, H, d] (ws_attn.cu; used by ws_unit.cu
+// for partial results that are merged afterwards).  Arguments and errors as ws_block_causal_attn with WS_DTYPE_BF16.
+int attn_bf16_in_f32_out(float* out, float* lse, const void* q, const void* k_cache, const void* v_cache, int64_t capacity,
+                         int64_t cache_len, const void* k_new, const void* v_new, int32_t Ln, int32_t H, int32_t d, int32_t Lq,
+                         const ws_block_mask* mask, float softmax_scale, void* workspace, size_t workspace_bytes, void* stream);
 int cache_write_validate(const void* k_cache, const void* v_cache, int64_t capacity, int32_t H, int32_t d, const void* k_src,
                          const void* v_src, int32_t n_rows, int32_t H_src, int32_t head_begin, int64_t row_offset, ws_dtype dt);
 

@@ -34,8 +34,8 @@ Staging staging_layout(int32_t Lq, int32_t Ln, int32_t H, int32_t d, int32_t n_s
   s.k_new = off; off = align_up(off + (size_t)n_steps * Ln * H * d * es, 256);
   s.v_new = off; off = align_up(off + (size_t)n_steps * Ln * H * d * es, 256);
   s.out = off; off = align_up(off + (size_t)n_steps * Lq * H * d * es, 256);
-  s.out_a = off; off = align_up(off + (size_t)Lq * H * d * es, 256);
-  s.out_b = off; off = align_up(off + (size_t)Lq * H * d * es, 256);
+  s.out_a = off; off = align_up(off + (size_t)Lq * H * d * 4, 256);  // the two partial results stay FP32 until they are merged
+  s.out_b = off; off = align_up(off + (size_t)Lq * H * d * 4, 256);
   s.lse_a = off; off = align_up(off + (size_t)Lq * H * 4, 256);
   s.lse_b = off; off = align_up(off + (size_t)Lq * H * 4, 256);
   s.attn_ws = off;
@@ -47,8 +47,10 @@ Staging staging_layout(int32_t Lq, int32_t Ln, int32_t H, int32_t d, int32_t n_s
 
 // out[i, h, :] = (w_a O_a[i, h, :] + w_b O_b[i, h, :]),  w_x = exp(lse_x[h, i] - logaddexp(lse_a, lse_b)[h, i]):
 // attention over the union of two disjoint key sets from the attention over each (natural-log LSE, [H, Lq]).
-// One thread per 8 elements (16 bytes).  A side whose LSE is -inf saw no key and gets weight 0.
-__global__ void __launch_bounds__(256) merge_two_kernel(uint4* __restrict__ out, const uint4* __restrict__ oa, const uint4* __restrict__ ob,
+// O_a, O_b are FP32 (the partial attentions' normalised rows before any rounding), so the merged row is rounded to
+// BF16 exactly once, like ws_block_causal_attn's.  One thread per 8 elements (two 16-byte loads per side, one 16-byte
+// store).  A side whose LSE is -inf saw no key and gets weight 0.
+__global__ void __launch_bounds__(256) merge_two_kernel(uint4* __restrict__ out, const float4* __restrict__ oa, const float4* __restrict__ ob,
                                                         const float* __restrict__ lse_a, const float* __restrict__ lse_b, int32_t Lq,
                                                         int32_t H, int32_t d8) {
   wsi::pdl_trigger();
@@ -65,17 +67,13 @@ __global__ void __launch_bounds__(256) merge_two_kernel(uint4* __restrict__ out,
     wa = ea * inv;
     wb = eb * inv;
   }
-  const uint4 a = oa[idx], b = ob[idx];
-  const uint32_t aw[4] = {a.x, a.y, a.z, a.w}, bw[4] = {b.x, b.y, b.z, b.w};
-  uint32_t r[4];
-#pragma unroll
-  for (int k = 0; k < 4; ++k) {
-    const float lo = wa * __uint_as_float(aw[k] << 16) + wb * __uint_as_float(bw[k] << 16);
-    const float hi = wa * __uint_as_float(aw[k] & 0xffff0000u) + wb * __uint_as_float(bw[k] & 0xffff0000u);
-    const __nv_bfloat162 p = __floats2bfloat162_rn(lo, hi);
-    r[k] = *reinterpret_cast<const uint32_t*>(&p);
-  }
-  out[idx] = make_uint4(r[0], r[1], r[2], r[3]);
+  const float4 a0 = oa[2 * idx], a1 = oa[2 * idx + 1], b0 = ob[2 * idx], b1 = ob[2 * idx + 1];
+  auto pack = [wa, wb](float ax, float bx, float ay, float by) {
+    const __nv_bfloat162 p = __floats2bfloat162_rn(wa * ax + wb * bx, wa * ay + wb * by);
+    return *reinterpret_cast<const uint32_t*>(&p);
+  };
+  out[idx] = make_uint4(pack(a0.x, b0.x, a0.y, b0.y), pack(a0.z, b0.z, a0.w, b0.w), pack(a1.x, b1.x, a1.y, b1.y),
+                        pack(a1.z, b1.z, a1.w, b1.w));
 }
 
 // Internal helper streams and events of ws_unit_forward_host (one set per device, created on first use).
@@ -186,23 +184,30 @@ extern "C" __attribute__((visibility("default"))) int ws_unit_forward_host(void*
     h2d(s.q + step * step_q, static_cast<const char*>(q_host) + step * step_q, step_q);
     inputs_arrived();
     if (e != cudaSuccess) break;
-    if (has_cache || !has_new)  // A: the cached keys (or, with no key at all, the zero / -inf result)
-      rc = ws_block_causal_attn(both ? st + s.out_a : out_s, both ? lse_a : nullptr, q_s, k_cache, v_cache, capacity, cache_len_after, nullptr,
-                                nullptr, 0, H, d, Lq, has_cache ? &mask_a : &mask_none, softmax_scale, st + s.attn_ws, s.attn_ws_bytes,
-                                WS_DTYPE_BF16, stream);
+    if (both)  // A: the cached keys, as an FP32 partial result
+      rc = wsi::attn_bf16_in_f32_out(reinterpret_cast<float*>(st + s.out_a), lse_a, q_s, k_cache, v_cache, capacity, cache_len_after, nullptr,
+                                     nullptr, 0, H, d, Lq, &mask_a, softmax_scale, st + s.attn_ws, s.attn_ws_bytes, stream);
+    else if (has_cache || !has_new)  // the cached keys are all there is (or, with no key at all, the zero / -inf result)
+      rc = ws_block_causal_attn(out_s, nullptr, q_s, k_cache, v_cache, capacity, cache_len_after, nullptr, nullptr, 0, H, d, Lq,
+                                has_cache ? &mask_a : &mask_none, softmax_scale, st + s.attn_ws, s.attn_ws_bytes, WS_DTYPE_BF16, stream);
     if (has_new && rc == WS_OK) {
       h2d(s.k_new + step * step_n, static_cast<const char*>(k_new_host) + step * step_n, step_n);
       h2d(s.v_new + step * step_n, static_cast<const char*>(v_new_host) + step * step_n, step_n);
       inputs_arrived();
       if (e != cudaSuccess) break;
       // B: the unit's own rows
-      rc = ws_block_causal_attn(both ? st + s.out_b : out_s, both ? lse_b : nullptr, q_s, k_cache, v_cache, capacity, 0,
-                                st + s.k_new + step * step_n, st + s.v_new + step * step_n, Ln, H, d, Lq, &mask_b, softmax_scale,
-                                st + s.attn_ws, s.attn_ws_bytes, WS_DTYPE_BF16, stream);
+      if (both)
+        rc = wsi::attn_bf16_in_f32_out(reinterpret_cast<float*>(st + s.out_b), lse_b, q_s, k_cache, v_cache, capacity, 0,
+                                       st + s.k_new + step * step_n, st + s.v_new + step * step_n, Ln, H, d, Lq, &mask_b, softmax_scale,
+                                       st + s.attn_ws, s.attn_ws_bytes, stream);
+      else
+        rc = ws_block_causal_attn(out_s, nullptr, q_s, k_cache, v_cache, capacity, 0, st + s.k_new + step * step_n,
+                                  st + s.v_new + step * step_n, Ln, H, d, Lq, &mask_b, softmax_scale, st + s.attn_ws, s.attn_ws_bytes,
+                                  WS_DTYPE_BF16, stream);
       if (both && rc == WS_OK) {
         const int64_t total = (int64_t)Lq * H * (d / 8);
         e = wsi::launch_pdl(merge_two_kernel, dim3((unsigned)((total + 255) / 256)), dim3(256), 0, stream, reinterpret_cast<uint4*>(out_s),
-                            reinterpret_cast<const uint4*>(st + s.out_a), reinterpret_cast<const uint4*>(st + s.out_b),
+                            reinterpret_cast<const float4*>(st + s.out_a), reinterpret_cast<const float4*>(st + s.out_b),
                             (const float*)lse_a, (const float*)lse_b, Lq, H, d / 8);
         if (e == cudaSuccess) wsi::count_launch(1);
       }

@@ -45,6 +45,39 @@ def ref_write(k_src, v_src, H, cap, hb, off, fill=(0xAB, 0xCD, 55, -66)):
     return kc8, vc8, ke, ve
 
 
+def test_fp8_cache_nan_source_is_contained_and_not_propagated():
+    """ws.h: FP8-cache sources must be finite.  What a NaN does is pinned here so that it cannot change unnoticed: the NaN
+    element is stored as the E4M3 NaN code (0x7f / 0xff), every OTHER (row, head) group is bit-exact as if the NaN were
+    not there, and ws_block_causal_attn_fp8kv does NOT hand the NaN on -- it reads the NaN code as a finite number (the
+    BF16 cache would return NaN rows).  Only the poisoned group's own exponent and codes are unspecified."""
+    n, H, d, cap = 64, 3, 128, 128
+    rng = np.random.default_rng(77)
+    k = wl.bf16_round(rng.standard_normal((n, H, d), dtype=np.float32))
+    v = wl.bf16_round(rng.standard_normal((n, H, d), dtype=np.float32))
+    tk, tv = to_dev(k, "bf16"), to_dev(v, "bf16")
+    tk[10, 1, 5] = float("nan")
+    tv[20, 2, 9] = float("nan")
+    kc8, vc8 = (torch.full((H, cap, d), 0xAB, dtype=torch.uint8, device="cuda") for _ in range(2))
+    ke, ve = (torch.full((H, cap), 55, dtype=torch.int8, device="cuda") for _ in range(2))
+    ws.kv_cache_write_fp8(kc8, vc8, ke, ve, tk, tv, 0, 0)
+    torch.cuda.synchronize()
+    want = ref_write(k, v, H, cap, 0, 0, fill=(0xAB, 0xAB, 55, 55))   # the oracle on the finite rows
+    for got, ref, (r, h, c) in ((kc8, want[0], (10, 1, 5)), (vc8, want[1], (20, 2, 9))):
+        g = got.cpu().numpy()
+        assert g[h, r, c] & 0x7f == 0x7f                     # the E4M3 NaN pattern
+        g[h, r, :] = ref[h, r, :]
+        assert np.array_equal(g, ref)                        # no other group is disturbed
+    for got, ref, (r, h) in ((ke, want[2], (10, 1)), (ve, want[3], (20, 2))):
+        g = got.cpu().numpy()
+        g[h, r] = ref[h, r]
+        assert np.array_equal(g, ref)
+    q = to_dev(wl.bf16_round(rng.standard_normal((40, H, d), dtype=np.float32)), "bf16")
+    out = torch.full_like(q, float("nan"))
+    ws.block_causal_attn_fp8kv(out, q, kc8, vc8, ke, ve, n, None, None, [40], [n], d ** -0.5, workspace_for(40, H, d, n))
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(out.float()).all())           # the documented hazard: a NaN in the source is silently finite here
+
+
 @pytest.mark.parametrize("n,Hs,d,H,cap,hb,off,spread", [
     (1024, 40, 128, 40, 2048, 0, 512, 0),     # cfg3's slice shape
     (257, 7, 128, 3, 1008, 2, 700, 3),        # head sub-range of a wider slice, ragged rows, rows of very different magnitude
