@@ -242,6 +242,41 @@ def test_fp8_attention_full_size_configs(name):
     assert q_err < 6e-2    # 4 significant bits: about 2^-5 per element, averaged over thousands of keys
 
 
+def test_fp8_attention_config5_step0_sampled():
+    """BASELINE.json config 5 (65536 cached rows, 970 x 40 x 128 queries) with the cache held in FP8 -- the launch bench.py times
+    in aux.fp8_kv_cache.cfg5.  The cache image (codes and exponents written by ws_kv_cache_write_fp8) is compared bit for bit with
+    the oracle's; the attention output of step 0 is compared on 1024 sampled (row, head) outputs that the oracle computes one by
+    one on the dequantised cache (full size -> sampled outputs), and the whole output must be written and in range."""
+    cfg = wl.CONFIGS["cfg5"]
+    x = wl.generate(cfg)
+    kc, vc = x["k_cache"].copy(), x["v_cache"].copy()
+    wsref.kv_cache_write(kc, vc, x["k_slice"], x["v_slice"], 0, cfg.write_offset)
+    Tc, H, d, cap = cfg.cache_len, cfg.H, cfg.d, cfg.capacity
+    k_rows = np.ascontiguousarray(np.transpose(kc[:, :Tc], (1, 0, 2)))
+    v_rows = np.ascontiguousarray(np.transpose(vc[:, :Tc], (1, 0, 2)))
+    del kc, vc
+    kc8, vc8, ke, ve = gpu_write(k_rows, v_rows, H, cap, 0, 0, fill=(0, 0, 0, 0))
+    w = ref_write(k_rows, v_rows, H, cap, 0, 0, fill=(0, 0, 0, 0))
+    del k_rows, v_rows
+    for g, ww, what in zip((kc8, vc8, ke, ve), w, ("k codes", "v codes", "k exponents", "v exponents")):
+        assert np.array_equal(g.cpu().numpy(), ww), f"cfg5 cache image, {what}"
+    kd, vd = wsref_fp8.kv_cache_dequant_fp8(w[0], w[2], Tc), wsref_fp8.kv_cache_dequant_fp8(w[1], w[3], Tc)
+    del w
+    q, kn, vn = x["q"][0], x["k_new"][0], x["v_new"][0]
+    tq, tkn, tvn = to_dev(q, "bf16"), to_dev(kn, "bf16"), to_dev(vn, "bf16")
+    out = torch.full_like(tq, float("nan"))
+    lse = torch.full((H, cfg.Lq), float("nan"), dtype=torch.float32, device="cuda")
+    wsp = workspace_for(cfg.Lq, H, d, Tc + cfg.Ln)
+    wsp.fill_(0xFF)
+    ws.block_causal_attn_fp8kv(out, tq, kc8, vc8, ke, ve, Tc, tkn, tvn, cfg.q_block_end, cfg.kv_visible, cfg.softmax_scale, wsp, lse=lse)
+    torch.cuda.synchronize()
+    got = to_host(out)
+    assert np.all(np.isfinite(got)) and np.abs(got).max() <= 4.0, "whole output must be written and inside the value range"
+    rows, heads = wl.sample_pairs(cfg, 1024)
+    ref, ref_lse = wsref.block_causal_attn_rows(q, kd, vd, Tc, kn, vn, cfg.q_block_end, cfg.kv_visible, cfg.softmax_scale, rows, heads)
+    check(got[rows, heads], lse.cpu().numpy()[heads, rows], ref, ref_lse, "cfg5 fp8 cache, step 0 (sampled)")
+
+
 def test_fp8_errors_leave_outputs_untouched():
     q = torch.zeros(64, 2, 128, dtype=torch.bfloat16, device="cuda")
     kc8 = torch.zeros(2, 256, 128, dtype=torch.uint8, device="cuda")

@@ -571,6 +571,32 @@ def test_unit_forward_host_two_steps_and_reuse_of_the_helper_streams():
         check_attn(got[s], ref, what=f"pipelined host entry step {s}")
 
 
+def test_unit_forward_host_is_as_accurate_as_the_single_pass_call():
+    """ws_unit_forward_host splits the keys by source (cache | the unit's own rows) and merges the two attentions by LSE.  The
+    partial results stay FP32 until the merge, so its output carries ONE rounding to BF16, like ws_block_causal_attn's: its
+    error against the oracle may not exceed the single-pass call's by more than a tenth, and the two GPU results agree far
+    inside the oracle tolerance (they differ by FP32 summation order and by which running maximum P was rounded against)."""
+    rng = np.random.default_rng(41)
+    H, d, Lq, Tc, cap = 6, 128, 300, 640, 640
+    r = lambda *s: wl.bf16_round(rng.standard_normal(s, dtype=np.float32))
+    k_cache, v_cache, q, kn, vn = r(H, cap, d), r(H, cap, d), r(1, Lq, H, d), r(1, Lq, H, d), r(1, Lq, H, d)
+    scale = 1.0 / math.sqrt(d)
+    host = lambda a: torch.from_numpy(wl.bf16_bits(a).view(np.int16)).view(torch.bfloat16).pin_memory()
+    kc, vc = to_dev(k_cache, "bf16"), to_dev(v_cache, "bf16")
+    outh = torch.zeros((1, Lq, H, d), dtype=torch.bfloat16).pin_memory()
+    staging = torch.empty(ws.unit_forward_host_staging_bytes(Lq, Lq, H, d, 0, Tc + Lq, 1), dtype=torch.uint8, device="cuda")
+    ws.unit_forward_host(outh, host(q), host(kn), host(vn), kc, vc, None, None, 0, Tc, scale, staging)
+    torch.cuda.synchronize()
+    got_host = wl.bf16_from_bits(outh.view(torch.int16).numpy().view(np.uint16))[0]
+    got_single, _ = gpu_attention(q[0], k_cache, v_cache, Tc, kn[0], vn[0], [Lq], [Tc + Lq], scale, want_lse=False)
+    ref, _ = wsref.block_causal_attn(q[0], k_cache, v_cache, Tc, kn[0], vn[0], [Lq], [Tc + Lq], scale)
+    _, rf_host = wsref.parity_metrics(got_host, ref)
+    _, rf_single = wsref.parity_metrics(got_single, ref)
+    ma_pair, rf_pair = wsref.parity_metrics(got_host, got_single.astype(np.float64))
+    assert rf_host <= 1.1 * rf_single + 2e-4, (rf_host, rf_single)
+    assert rf_pair <= 4e-3 and ma_pair <= 4e-3, (ma_pair, rf_pair)
+
+
 def test_fused_relayout_attention_in_fp32():
     """Config-1 arithmetic (FP32 in, rounded to BF16 on the device, FP32 out) through the token-major call:
     the staging cast gathers the rank's heads token by token."""
